@@ -1,0 +1,527 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (no GPU, no CUDA path).
+
+Each test names the pin of DESIGN.md / SURVEY.md section 8(c) it implements and the passage it rests on.
+Nothing here retypes the oracle's formulas: expectations come from the paper's printed values
+(tests/golden/), closed forms (DFT symbols of circulant operators, Eq. 17), invariants, exact
+rational arithmetic, or brute force with 2x2 complex matrices.
+"""
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+from conftest import read_golden
+from oracle import cosenu_ref as R
+from paper_2203_12866_b200 import inputs
+
+FD, FV = R.FD4_KO3, R.FV_WENO7
+
+
+def _fr(tok):
+    return [Fraction(t) for t in tok.split()]
+
+
+# ----------------------------------------------------------------------------- helpers
+def pvec(st, s):
+    """Polarization components of species s from the canonical state (Eq. 4)."""
+    o = 4 * s
+    return st[o] + st[o + 1], np.stack([2 * st[o + 2], -2 * st[o + 3], st[o] - st[o + 1]])
+
+
+def state_from_pvec(P0, P):
+    ee = 0.5 * (P0 + P[2]); xx = 0.5 * (P0 - P[2])
+    return ee, xx, 0.5 * P[0], -0.5 * P[1]
+
+
+def rk4_poly(x):
+    return 1 + x + x * x / 2 + x ** 3 / 6 + x ** 4 / 24
+
+
+def linear_closed_form(st0, nsteps, dt, omega, theta, lam_adv):
+    """Exact n-step RK4 evolution of the mu=0 system for a circulant advection operator.
+
+    lam_adv[k, j]: eigenvalue of the semi-discrete advection operator on exp(i 2 pi k z_i/L) for
+    beam j.  Flavour part: dP/dt = omega B x P, B = (sin 2theta, 0, -cos 2theta) (Eq. 1 + H_vac,
+    PAPER.md:41-66), whose eigen-components are P0, P.B (eigenvalue 0) and
+    c = P.e1 + i P.(B x e1) (eigenvalue +i omega).  Advection and rotation commute, so each Fourier
+    mode of each eigen-component is multiplied by R(dt (lam + g))^n.
+    """
+    B = np.array([np.sin(2 * theta), 0.0, -np.cos(2 * theta)])
+    e1 = np.array([0.0, 1.0, 0.0]); e2 = np.cross(B, e1)
+    m0 = rk4_poly(dt * lam_adv) ** nsteps
+    m1 = rk4_poly(dt * (lam_adv + 1j * omega)) ** nsteps
+    out = np.empty_like(st0)
+    for s in range(2):
+        P0, P = pvec(st0, s)
+        par = np.tensordot(B, P, axes=(0, 0))
+        c = np.tensordot(e1, P, axes=(0, 0)) + 1j * np.tensordot(e2, P, axes=(0, 0))
+        P0n = np.fft.ifft(np.fft.fft(P0, axis=0) * m0, axis=0).real
+        parn = np.fft.ifft(np.fft.fft(par, axis=0) * m0, axis=0).real
+        cn = np.fft.ifft(np.fft.fft(c, axis=0) * m1, axis=0)
+        Pn = (B[:, None, None] * parn[None] + e1[:, None, None] * cn.real[None] + e2[:, None, None] * cn.imag[None])
+        ee, xx, r, im = state_from_pvec(P0n, Pn)
+        out[4 * s], out[4 * s + 1], out[4 * s + 2], out[4 * s + 3] = ee, xx, r, im
+    return out
+
+
+def fd_ko_symbol(nz, nv, dz, eps_ko):
+    th = 2 * np.pi * np.fft.fftfreq(nz)[:, None]  # k dz
+    v = inputs.v_grid(nv)[None, :]
+    return -1j * v * (8 * np.sin(th) - np.sin(2 * th)) / (6 * dz) - (eps_ko / dz) * np.sin(th / 2) ** 4
+
+
+def weno_linear_symbol(nz, nv, dz):
+    a = [float(x) for x in _fr(read_golden("paper_appendix_a.txt")["A1"])]  # Eq. (A.1) as printed
+    th = 2 * np.pi * np.fft.fftfreq(nz)[:, None]
+    v = inputs.v_grid(nv)[None, :]
+    pos = sum(a[m + 3] * np.exp(1j * m * th) for m in range(-3, 4))
+    neg = sum(a[m + 3] * np.exp(1j * (1 - m) * th) for m in range(-3, 4))
+    sym = np.where(v >= 0, pos, neg)
+    return -(v / dz) * (1 - np.exp(-1j * th)) * sym
+
+
+# ----------------------------------------------------------------------------- P5: App. A constants
+def test_P5_weno_constants_exact_rationals():
+    """sum_r d_r (A.2)_r == (A.1) with the oracle's d_r and candidates."""
+    gold = read_golden("paper_appendix_a.txt")
+    a1 = _fr(gold["A1"])
+    left = [int(x) for x in gold["S_left"].split()]
+    # oracle's candidate coefficients, extracted by feeding unit vectors
+    C = np.zeros((4, 7))
+    for m in range(7):
+        e = np.zeros(7); e[m] = 1.0
+        C[:, m] = R.weno7_candidates(e)
+    for r in range(4):
+        want = [Fraction(0)] * 7
+        for q, coef in enumerate(_fr(gold["A2_r%d" % r])):
+            want[3 + left[r] + q] = coef
+        assert np.allclose(C[r], [float(x) for x in want], rtol=0, atol=1e-16), r
+    d = R.weno7_dr()
+    dq = [Fraction(x).limit_denominator(1000) for x in d]
+    assert [float(x) for x in dq] == list(d)
+    # exact identity in rationals with the paper's A.2 and the oracle's d_r
+    comb = [Fraction(0)] * 7
+    for r in range(4):
+        for q, coef in enumerate(_fr(gold["A2_r%d" % r])):
+            comb[3 + left[r] + q] += dq[r] * coef
+    assert comb == a1
+    # reading A6: the printed list is the same set in reverse order, and as printed it does NOT
+    # reproduce (A.1)
+    printed = _fr(gold["d_printed"])
+    assert dq == printed[::-1]
+    comb_p = [Fraction(0)] * 7
+    for r in range(4):
+        for q, coef in enumerate(_fr(gold["A2_r%d" % r])):
+            comb_p[3 + left[r] + q] += printed[r] * coef
+    assert comb_p != a1
+    assert sum(dq) == 1
+
+
+def test_P5_smoothness_indicator_properties():
+    """SI_r(const)=0, SI_r(unit slope)=240, SI >= 0, mirror symmetry SI0<->SI3, SI1<->SI2 (A.3)."""
+    assert np.all(R.weno7_si(np.ones(7)) == 0)
+    assert np.allclose(R.weno7_si(np.arange(7.0)), 240.0, rtol=1e-12)
+    assert np.allclose(R.weno7_si(np.arange(7.0) * 0.5 + 3), 60.0, rtol=1e-9)  # quadratic scaling
+    rng = np.random.default_rng(5)
+    for _ in range(200):
+        f = rng.standard_normal(7)
+        si = R.weno7_si(f)
+        assert np.all(si >= -1e-9 * np.abs(f).max() ** 2)
+        assert np.allclose(si, R.weno7_si(f[::-1])[::-1], rtol=1e-12, atol=1e-10)
+    # each SI_r only sees its own sub-stencil S_r
+    left = [0, -1, -2, -3]
+    base = rng.standard_normal(7)
+    for r in range(4):
+        for m in range(7):
+            f = base.copy(); f[m] += 1.0
+            changed = R.weno7_si(f)[r] != R.weno7_si(base)[r]
+            assert changed == (3 + left[r] <= m <= 3 + left[r] + 3)
+    # Jiang-Shu integral: 240 * sum_l int dz^(2l-1) (p^(l))^2 over cell i for the cubic through S_r
+    # (SURVEY A7); check on a quadratic f = z^2 cell averages, brute-force polynomial integration
+    from numpy.polynomial import polynomial as Pn
+    for r in range(4):
+        cells = np.arange(left[r], left[r] + 4)
+        vals = rng.standard_normal(4)
+        # cubic p whose cell averages over [c-1/2, c+1/2] equal vals
+        A = np.array([[((c + .5) ** (q + 1) - (c - .5) ** (q + 1)) / (q + 1) for q in range(4)] for c in cells])
+        coef = np.linalg.solve(A, vals)
+        tot = 0.0
+        for l in (1, 2, 3):
+            dcoef = Pn.polyder(coef, l)
+            sq = Pn.polyint(Pn.polymul(dcoef, dcoef))
+            tot += Pn.polyval(0.5, sq) - Pn.polyval(-0.5, sq)
+        f = np.zeros(7); f[3 + left[r]: 3 + left[r] + 4] = vals
+        assert np.isclose(R.weno7_si(f)[r], 240 * tot, rtol=1e-10)
+
+
+def test_weno_face_is_convex_combination_and_7th_order():
+    """Eq. (13,14): smooth data -> weights ~ d_r -> 7th-order value."""
+    rng = np.random.default_rng(1)
+    for _ in range(50):
+        f = rng.standard_normal(7)
+        F = R.weno7_face(f, 1e-6)
+        c = R.weno7_candidates(f)
+        assert c.min() - 1e-12 <= F <= c.max() + 1e-12
+    # cell averages of sin on a fine grid: error of the face value ~ h^7 for eps >> SI
+    errs = []
+    for h in (0.2, 0.1):
+        x = (np.arange(-3, 4)) * h + 0.3
+        avg = (np.cos(x - h / 2) - np.cos(x + h / 2)) / h
+        errs.append(abs(R.weno7_face(avg, 1e30) - np.sin(0.3 + h / 2)))
+    assert 6.5 < np.log2(errs[0] / errs[1]) < 7.5
+
+
+# ----------------------------------------------------------------------------- v-grid pin
+def test_v_grid_bin_centres():
+    """PAPER.md:78 + the printed beam v_z = 0.99 at N_v = 100."""
+    g = read_golden("paper_values.txt")
+    nv = int(g["nv_fiducial"])
+    sim = R.RefSim(16, nv, 16.0, 0.1, 0.0, 0.0, 0.0, FD)
+    # advect a state that is 1 in component 0 with a linear-in-z... simpler: read v from the FD
+    # response to u = sin(2 pi z/L): k = -v * d/dz u (KO off)
+    sim.set_option(R.OPT_EPS_KO, 0.0)
+    nz = 16; z = np.arange(nz)
+    st = np.zeros((8, nz, nv)); st[0] = np.sin(2 * np.pi * z / nz)[:, None]
+    k = sim.rhs(st)[0]
+    th = 2 * np.pi / nz
+    deriv = (8 * np.sin(th) - np.sin(2 * th)) / 6 * np.cos(2 * np.pi * z / nz)
+    v = -(k * deriv[:, None]).sum(0) / (deriv ** 2).sum()
+    assert np.allclose(v, inputs.v_grid(nv), atol=1e-13)
+    assert np.isclose(v[-1], float(g["v_beam_fiducial"]), atol=1e-13)
+    assert np.isclose(v[0], -float(g["v_beam_fiducial"]), atol=1e-13)
+
+
+# ----------------------------------------------------------------------------- P1: Eq. (17)
+@pytest.mark.parametrize("scheme", [FD, FV])
+def test_P1_vacuum_solution_eq17_uniform(scheme):
+    """Eq. (17a-d) for a z-uniform pure nu_e state, nu and nubar, every step."""
+    g = read_golden("paper_values.txt")
+    om = float(g["omega_vac"]); th = np.deg2rad(float(g["theta_vac_deg"]))
+    nz, nv, dt = 16, 2, 0.05
+    sim = R.RefSim(nz, nv, 16.0, dt, om, th, 0.0, scheme)
+    st = np.zeros((8, nz, nv)); st[0] = 1.0; st[4] = 0.7
+    sim.set_state(st)
+    s2, c2 = np.sin(2 * th), np.cos(2 * th)
+    minee = 1.0
+    for n in range(1, 1400):
+        sim.step(1)
+        t = n * dt
+        y = sim.get_state()
+        ss = np.sin(om * t / 2) ** 2
+        want = [1 - s2 * s2 * ss, s2 * s2 * ss, -s2 * c2 * ss, 0.5 * s2 * np.sin(om * t)]
+        if n % 50 == 0 or n < 5:
+            for c in range(4):
+                assert np.allclose(y[c], want[c], rtol=0, atol=2e-10), (n, c)
+                assert np.allclose(y[4 + c], 0.7 * want[c], rtol=0, atol=2e-10), (n, c)
+        minee = min(minee, y[0].min())
+    # the printed minimum of <rho_ee>, to its three printed decimals
+    assert abs(minee - float(g["min_rho_ee_theta37"])) < 5e-4
+    assert abs(minee - (1 - s2 * s2)) < 1e-5
+
+
+@pytest.mark.parametrize("scheme", [FD, FV])
+def test_P1_vacuum_solution_eq17_travelling_gaussian(scheme):
+    """Eq. (17) with the advected profile rho_ee^{t0}(z - v t), v = +-0.5."""
+    g = read_golden("paper_values.txt")
+    om = float(g["omega_vac"]); th = np.deg2rad(float(g["theta_vac_deg"]))
+    nz, nv, L = 240, 2, 240.0
+    dt = 0.2 * 1.0 / 0.5
+    assert np.allclose(np.abs(inputs.v_grid(nv)), float(g["v_beam"]))
+    sim = R.RefSim(nz, nv, L, dt, om, th, 0.0, scheme, eps_ko=0.0)
+    z = np.arange(nz) * 1.0
+    prof = lambda x: np.exp(-((x - L / 2 + L / 2) % L - L / 2) ** 2 / (2 * 20.0 ** 2))
+    st = np.zeros((8, nz, nv)); st[0] = prof(z)[:, None]; st[4] = st[0]
+    sim.set_state(st)
+    nsteps = 150
+    sim.step(nsteps)
+    t = nsteps * dt
+    y = sim.get_state()
+    s2, c2 = np.sin(2 * th), np.cos(2 * th)
+    ss = np.sin(om * t / 2) ** 2
+    for j, v in enumerate(inputs.v_grid(nv)):
+        sh = prof(z - v * t)
+        want = [sh * (1 - s2 * s2 * ss), sh * s2 * s2 * ss, -sh * s2 * c2 * ss, 0.5 * sh * s2 * np.sin(om * t)]
+        for c in range(4):
+            assert np.abs(y[c, :, j] - want[c]).max() < 2e-5, (j, c)
+            assert np.abs(y[4 + c, :, j] - want[c]).max() < 2e-5, (j, c)
+    d = sim.diagnostics()
+    assert abs(d["psurv_nu"] - (1 - s2 * s2 * ss)) < 1e-6  # <rho_ee>(t)
+
+
+# ----------------------------------------------------------------------------- P2: |P|, P0
+def test_P2_norm_and_trace_under_commutator():
+    """|P| and P0 are constants of motion of the commutator; drift is O(dt^4)."""
+    nz, nv = 16, 6
+    rng = np.random.default_rng(3)
+    col = rng.uniform(-0.5, 0.5, (8, 1, nv))
+    st = np.repeat(col, nz, axis=1)  # z-uniform => no advection (P8)
+    drifts = []
+    for dt in (0.1, 0.05):
+        sim = R.RefSim(nz, nv, 16.0, dt, 0.3, 0.2, 1.5, FD)
+        sim.set_state(st)
+        sim.step(int(round(4.0 / dt)))
+        y = sim.get_state()
+        worst = 0.0
+        for s in range(2):
+            P0a, Pa = pvec(st, s); P0b, Pb = pvec(y, s)
+            assert np.abs(P0a - P0b).max() < 1e-14
+            worst = max(worst, np.abs(np.linalg.norm(Pa, axis=0) - np.linalg.norm(Pb, axis=0)).max())
+        drifts.append(worst)
+    assert drifts[0] < 1e-4 and drifts[1] < drifts[0] / 12  # ~ dt^4 (ratio 16) with slack
+
+
+# ----------------------------------------------------------------------------- P3 / P4: FD + KO closed form
+@pytest.mark.parametrize("omega,theta", [(0.0, 0.0), (1.0, 0.1), (0.7, np.deg2rad(37))])
+def test_P3_fd_ko_discrete_closed_form(omega, theta):
+    """FD4 + KO3 + RK4 with mu=0 equals the DFT closed form to rounding, for white-noise data."""
+    nz, nv, dt, nsteps = 96, 6, 0.4, 100
+    st = inputs.random_state(nz, nv, 77)
+    sim = R.RefSim(nz, nv, float(nz), dt, omega, theta, 0.0, FD)
+    sim.set_state(st); sim.step(nsteps)
+    want = linear_closed_form(st, nsteps, dt, omega, theta, fd_ko_symbol(nz, nv, 1.0, 0.1))
+    assert np.abs(sim.get_state() - want).max() < 5e-14
+
+
+def test_P3_fd_coefficients_without_ko_and_dz_scaling():
+    nz, nv, dt, nsteps, L = 64, 4, 0.1, 40, 32.0
+    st = inputs.random_state(nz, nv, 78)
+    sim = R.RefSim(nz, nv, L, dt, 0.0, 0.0, 0.0, FD, eps_ko=0.0)
+    sim.set_state(st); sim.step(nsteps)
+    want = linear_closed_form(st, nsteps, dt, 0.0, 0.0, fd_ko_symbol(nz, nv, L / nz, 0.0))
+    assert np.abs(sim.get_state() - want).max() < 5e-14
+
+
+def test_P4_ko_damps_nyquist_mode():
+    """KO alone on u_i = (-1)^i: semi-discrete decay exp(-eps t/dz) (reading A4: dissipative sign)."""
+    nz, nv, eps = 32, 2, 0.1
+    sim = R.RefSim(nz, nv, float(nz), 0.01, 0.0, 0.0, 0.0, FD, eps_ko=eps)
+    st = np.zeros((8, nz, nv)); st[0] = ((-1.0) ** np.arange(nz))[:, None]
+    k = sim.rhs(st)[0]
+    # FD4 annihilates the Nyquist mode, so k = Q u = -(eps/dz) u exactly
+    assert np.allclose(k, -eps * st[0], atol=1e-15)
+    sim.set_state(st); sim.step(500)
+    assert np.allclose(sim.get_state()[0], st[0] * np.exp(-eps * 5.0), rtol=1e-9)
+
+
+# ----------------------------------------------------------------------------- P6: WENO linear limit
+@pytest.mark.parametrize("omega,theta", [(0.0, 0.0), (1.0, 0.1)])
+def test_P6_weno_linear_limit_closed_form(omega, theta):
+    """eps -> 1e30 turns Alg. 1 into the linear scheme (A.1); flux-difference form + upwinding (A9)."""
+    nz, nv, dt, nsteps = 64, 6, 0.4, 60
+    st = inputs.random_state(nz, nv, 79)
+    sim = R.RefSim(nz, nv, float(nz), dt, omega, theta, 0.0, FV, weno_eps=1e30)
+    sim.set_state(st); sim.step(nsteps)
+    want = linear_closed_form(st, nsteps, dt, omega, theta, weno_linear_symbol(nz, nv, 1.0))
+    assert np.abs(sim.get_state() - want).max() < 5e-14
+
+
+def test_weno_upwinding_is_stable_and_mirror_symmetric():
+    """Reading A9: errors for +v and -v are mirror images; amplitude never grows."""
+    nz, nv = 64, 2
+    z = np.arange(nz)
+    prof = np.exp(-((z - 32.0) / 5.0) ** 2)
+    st = np.zeros((8, nz, nv)); st[0, :, 0] = prof[::-1]; st[0, :, 1] = prof
+    sim = R.RefSim(nz, nv, float(nz), 0.4, 0.0, 0.0, 0.0, FV)
+    sim.set_state(st); sim.step(100)
+    y = sim.get_state()[0]
+    assert np.allclose(y[:, 0], y[::-1, 1], atol=1e-13)
+    assert np.abs(y).max() <= 1.0 + 1e-12
+    assert np.isclose(y[:, 1].sum(), prof.sum(), rtol=1e-13)  # conservation (telescoping fluxes)
+
+
+# ----------------------------------------------------------------------------- P7: convergence orders
+def _advection_error(scheme, nz, eps_ko=None, weno_eps=None, T=2.0):
+    """E2 (Eq. 15) of pure advection (mu=omega=0) of a smooth periodic profile."""
+    nv, L = 2, 2 * np.pi
+    dz = L / nz
+    nsteps = int(np.ceil(T / (0.02 * dz))); dt = T / nsteps  # tiny dt: the spatial error dominates
+    sim = R.RefSim(nz, nv, L, dt, 0.0, 0.0, 0.0, scheme, eps_ko=eps_ko, weno_eps=weno_eps)
+    if scheme == FV:  # cell averages of exp(sin z) are not closed-form: use sin (A13: averages)
+        zl = np.arange(nz) * dz
+        f0 = lambda x: (np.cos(x) - np.cos(x + dz)) / dz  # average of sin over [x, x+dz]
+        exact = lambda v: f0(zl - v * T)
+        init = f0(zl)
+    else:
+        zl = np.arange(nz) * dz
+        exact = lambda v: np.sin(zl - v * T)
+        init = np.sin(zl)
+    st = np.zeros((8, nz, nv)); st[0] = init[:, None]
+    sim.set_state(st); sim.step(nsteps)
+    y = sim.get_state()[0]
+    v = inputs.v_grid(nv)
+    return max(np.sqrt(np.mean((y[:, j] - exact(v[j])) ** 2)) for j in range(nv))
+
+
+def test_P7_convergence_orders():
+    """FD4 -> 4; KO3(0.1) lowers it (-> 3); WENO7 -> 7 in its linear limit, ~6-7 with
+    eps = 1e-6 on a sinusoid (order loss at critical points is a property of the weights)."""
+    g = read_golden("paper_values.txt")
+    e = [_advection_error(FD, n, eps_ko=0.0) for n in (16, 32)]
+    assert abs(np.log2(e[0] / e[1]) - float(g["order_fd4"])) < 0.25
+    e = [_advection_error(FD, n, eps_ko=0.1) for n in (64, 128)]
+    assert 2.7 < np.log2(e[0] / e[1]) < 3.3
+    e = [_advection_error(FV, n, weno_eps=1e30) for n in (16, 32)]
+    assert abs(np.log2(e[0] / e[1]) - float(g["order_weno7"])) < 0.4
+    e = [_advection_error(FV, n, weno_eps=1e-6) for n in (16, 32)]
+    assert 5.0 < np.log2(e[0] / e[1]) < 8.5
+
+
+# ----------------------------------------------------------------------------- P8: uniform state
+@pytest.mark.parametrize("scheme", [FD, FV])
+def test_P8_uniform_state_has_zero_advection(scheme):
+    nz, nv = 16, 5  # odd nv: includes the v = 0 beam
+    rng = np.random.default_rng(8)
+    st = np.repeat(rng.uniform(0.1, 1.0, (8, 1, nv)), nz, axis=1)
+    sim = R.RefSim(nz, nv, 16.0, 0.1, 0.0, 0.0, 0.0, scheme)
+    k = sim.rhs(st)
+    assert np.abs(k).max() <= 4e-16 * np.abs(st).max() * 25
+
+
+# ----------------------------------------------------------------------------- P9: brute force
+def _brute_force_commutator(st, omega, theta, mu):
+    """Eq. (1), (3a), (3b) with 2x2 complex matrices and the direct double sum."""
+    _, nz, nv = st.shape
+    v = inputs.v_grid(nv); dv = 2.0 / nv
+    Hv = 0.5 * omega * np.array([[-np.cos(2 * theta), np.sin(2 * theta)], [np.sin(2 * theta), np.cos(2 * theta)]])
+    out = np.zeros_like(st)
+    for i in range(nz):
+        rho = [np.array([[st[0, i, j], st[2, i, j] + 1j * st[3, i, j]],
+                         [st[2, i, j] - 1j * st[3, i, j], st[1, i, j]]]) for j in range(nv)]
+        rhob = [np.array([[st[4, i, j], st[6, i, j] + 1j * st[7, i, j]],
+                          [st[6, i, j] - 1j * st[7, i, j], st[5, i, j]]]) for j in range(nv)]
+        for j in range(nv):
+            H = Hv.astype(complex).copy(); Hb = Hv.astype(complex).copy()
+            for jp in range(nv):
+                w = dv * (1 - v[j] * v[jp])
+                H += mu * w * (rho[jp] - np.conj(rhob[jp]))      # Eq. (3a); alpha folded into rho_bar
+                Hb -= mu * w * (np.conj(rho[jp]) - rhob[jp])     # Eq. (3b)
+            d = -1j * (H @ rho[j] - rho[j] @ H)
+            db = -1j * (Hb @ rhob[j] - rhob[j] @ Hb)
+            for o, m in ((0, d), (4, db)):
+                assert abs(m[0, 0].imag) < 1e-12 and abs(m[1, 0] - np.conj(m[0, 1])) < 1e-12
+                out[o, i, j] = m[0, 0].real; out[o + 1, i, j] = m[1, 1].real
+                out[o + 2, i, j] = m[0, 1].real; out[o + 3, i, j] = m[0, 1].imag
+    return out
+
+
+@pytest.mark.parametrize("nv", [2, 3, 4])
+def test_P9_commutator_and_moments_brute_force(nv):
+    nz = 16
+    st = inputs.random_state(nz, nv, 100 + nv)
+    for (om, th, mu) in ((0.0, 0.0, 1.0), (0.4, 0.3, 0.0), (0.4, 0.3, 2.5)):
+        sim = R.RefSim(nz, nv, 16.0, 0.1, om, th, mu, FD, advect=False)
+        k = sim.rhs(st)
+        want = _brute_force_commutator(st, om, th, mu)
+        assert np.abs(k - want).max() < 5e-15 * max(1.0, mu) * 10
+    # the 6 moments against the plain sums
+    M = R.RefSim(nz, nv, 16.0, 0.1, 0, 0, 1.0, FD).moments(st)
+    v = inputs.v_grid(nv); dv = 2.0 / nv
+    Dd = (st[0] - st[1]) - (st[4] - st[5]); Dr = st[2] - st[6]; Di = st[3] + st[7]
+    for q, X in enumerate((Dd, Dr, Di)):
+        assert np.allclose(M[2 * q], dv * X.sum(1), atol=1e-15)
+        assert np.allclose(M[2 * q + 1], dv * (X * v).sum(1), atol=1e-15)
+
+
+def test_rhs_is_advection_plus_commutator():
+    """Eq. (1): the two terms add; checks the ADVECT test hook does not change the commutator."""
+    nz, nv = 32, 4
+    st = inputs.random_state(nz, nv, 5)
+    for scheme in (FD, FV):
+        full = R.RefSim(nz, nv, 32.0, 0.1, 0.3, 0.2, 1.0, scheme).rhs(st)
+        comm = R.RefSim(nz, nv, 32.0, 0.1, 0.3, 0.2, 1.0, scheme, advect=False).rhs(st)
+        adv = R.RefSim(nz, nv, 32.0, 0.1, 0.0, 0.0, 0.0, scheme).rhs(st)
+        assert np.abs(full - (comm + adv)).max() < 1e-14 * 50
+
+
+# ----------------------------------------------------------------------------- P10 / P11
+@pytest.mark.parametrize("scheme", [FD, FV])
+def test_P10_M0_conservation(scheme):
+    """Eq. (19): M0 conserved for omega=0 with periodic BC, to rounding."""
+    nz, nv = 64, 8
+    sim = R.RefSim(nz, nv, 64.0, 0.4, 0.0, 0.0, 1.0, scheme)
+    sim.init(4242, pert_amp=1e-2)
+    d0 = sim.diagnostics()
+    assert np.isclose(d0["M0"][2], (1 - 0.9) * 64.0, rtol=1e-13)  # (1-alpha) L  (A14)
+    sim.step(200)
+    d = sim.diagnostics()
+    assert d["ex_abs_max"] > 1e-2  # the run is not trivial
+    assert max(abs(x) for x in d["dM0"]) < 1e-12 * abs(d0["M0"][2])
+    # omega != 0: only B.M0 is conserved
+    th = 0.3
+    sim = R.RefSim(nz, nv, 64.0, 0.4, 0.2, th, 1.0, scheme)
+    sim.init(4242, pert_amp=1e-2); sim.step(100)
+    d = sim.diagnostics()
+    B = np.array([np.sin(2 * th), 0, -np.cos(2 * th)])
+    assert abs(B @ np.array(d["dM0"])) < 1e-12 * 6.4
+    assert np.abs(d["dM0"]).max() > 1e-6
+
+
+@pytest.mark.parametrize("scheme", [FD, FV])
+def test_P11_symmetric_manifold(scheme):
+    """omega=0 and rho_bar(0) = c rho^*(0): stays so, since rho_bar^* obeys rho's equation (H_bar = -H^*)."""
+    nz, nv, c = 32, 6, 0.8
+    st = inputs.smooth_random_state(nz, nv, 9)
+    st[4], st[5], st[6], st[7] = c * st[0], c * st[1], c * st[2], -c * st[3]
+    # WENO's fixed eps is not scale invariant (weights of c*u differ from those of u at O(eps/SI)),
+    # so the FV case is run in its linear limit; the property pinned here is the H_bar reading.
+    sim = R.RefSim(nz, nv, 32.0, 0.2, 0.0, 0.0, 1.3, scheme, weno_eps=1e30)
+    sim.set_state(st); sim.step(50)
+    y = sim.get_state()
+    assert np.abs(y - st).max() > 1e-3
+    for a, b, sgn in ((0, 4, 1), (1, 5, 1), (2, 6, 1), (3, 7, -1)):
+        assert np.abs(y[b] - sgn * c * y[a]).max() < 1e-13
+
+
+# ----------------------------------------------------------------------------- init + diagnostics + ABI
+def test_init_matches_input_recipe_and_is_normalised():
+    nz, nv = 64, 16
+    for seed in (1, 12866):
+        sim = R.RefSim(nz, nv, 64.0, 0.4, 0.0, 0.0, 1.0, FD)
+        sim.init(seed)
+        a = sim.get_state(); b = inputs.fast_conversion_state(nz, nv, seed)
+        assert np.abs(a - b).max() < 1e-15
+        dv = 2.0 / nv
+        assert np.isclose(a[0, 0].sum() * dv, 1.0, rtol=1e-15)
+        assert np.isclose(a[4, 0].sum() * dv, 0.9, rtol=1e-15)
+        # more forward-peaked nubar (sigma 0.5 < 0.6): ELN crossing exists
+        G = a[0, 0] - a[4, 0]
+        assert G.min() < 0 < G.max()
+    # pert kinds 1, 2 run and keep |rho_ex| at the requested scale
+    for kind, amp in ((1, 1e-6), (2, 1e-2)):
+        sim = R.RefSim(nz, nv, 64.0, 0.4, 0.0, 0.0, 1.0, FV)
+        sim.init(3, pert_amp=amp, pert_kind=kind)
+        d = sim.diagnostics()
+        assert 0 < d["ex_abs_max"] < 10 * amp
+        assert d["dP_max"] < 1e-12 or kind == 1
+
+
+def test_diagnostics_definitions():
+    """psurv, dP (Eq. 22, 23), M0 (Eq. 19) on a hand-built state."""
+    nz, nv = 16, 2
+    sim = R.RefSim(nz, nv, 8.0, 0.1, 0.0, 0.0, 0.0, FD)
+    st = np.zeros((8, nz, nv)); st[0] = 1.0; st[4] = 0.5
+    sim.set_state(st)
+    d = sim.diagnostics()
+    assert d["psurv_nu"] == 1.0 and d["dP_max"] == 0.0 and d["dP_avg"] == 0.0
+    assert np.allclose(d["M0"], [0, 0, 0.5 * 8.0 * 2.0])  # int dz int dv (1 - 0.5)
+    st2 = st.copy(); st2[0, 3, 1] = 0.5; st2[1, 3, 1] = 0.5  # one cell fully mixed: |P| = 0 there
+    sim2 = R.RefSim(nz, nv, 8.0, 0.1, 0.0, 0.0, 0.0, FD)
+    sim2.set_state(st2)
+    d2 = sim2.diagnostics()
+    assert np.isclose(d2["psurv_nu"], 1.0)
+    # |P| reference is the z-mean at t=0: (15*1 + 0)/16 for beam 1
+    assert np.isclose(d2["dP_max"], 1.0)  # the mixed cell has |P| = 0 -> |0/ref - 1| = 1
+
+
+def test_abi_argument_validation():
+    L = R.lib()
+    assert not L.cosenu_ref_create(8, 4, 1.0, 0.1, 0, 0, 0, 0)       # nz < 16
+    assert not L.cosenu_ref_create(16, 1, 1.0, 0.1, 0, 0, 0, 0)      # nv < 2
+    assert not L.cosenu_ref_create(16, 4, -1.0, 0.1, 0, 0, 0, 0)
+    assert not L.cosenu_ref_create(16, 4, 1.0, 0.0, 0, 0, 0, 0)
+    assert not L.cosenu_ref_create(16, 4, 1.0, 0.1, 0, 0, 0, 7)
+    assert L.cosenu_ref_last_error(None)
+    sim = R.RefSim(16, 4, 1.0, 0.1, 0, 0, 0, 0)
+    assert L.cosenu_ref_step(sim.h, 1) == 4  # ESTATE before init
+    with pytest.raises(RuntimeError):
+        sim.set_option(99, 1.0)
