@@ -1,0 +1,178 @@
+"""Thin Python binding over the C ABI of include/cosenu.h (argument marshalling only).
+
+Every step of the path runs in the CUDA kernels of csrc/.  PyTorch is used for the device workspace
+(`torch.empty(..., device='cuda')`) and the stream.  There is NO CPU fallback: if the CUDA library is
+missing or no sm_100 device is present, loading / `Cosenu(...)` raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libcosenu_b200.so")
+
+FD4_KO3, FV_WENO7 = 0, 1
+OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, 1, 2, 3, 4
+OPT_EPS_KO, OPT_WENO_EPS, OPT_ADVECT, OPT_LEAN_ACC, OPT_STAGE_TIMING = 0, 1, 2, 3, 4
+
+# every symbol include/cosenu.h declares
+SYMBOLS = ["cosenu_create", "cosenu_workspace_bytes", "cosenu_attach", "cosenu_set_option", "cosenu_init",
+           "cosenu_set_state", "cosenu_step", "cosenu_get_state", "cosenu_get_moments", "cosenu_diagnostics",
+           "cosenu_sync", "cosenu_launch_count", "cosenu_stage_times", "cosenu_destroy", "cosenu_last_error"]
+
+
+class Diag(C.Structure):
+    _fields_ = [("t", C.c_double), ("step", C.c_int64),
+                ("psurv_nu", C.c_double), ("psurv_nubar", C.c_double),
+                ("dP_max", C.c_double), ("dP_avg", C.c_double),
+                ("M0", C.c_double * 3), ("dM0", C.c_double * 3),
+                ("trace_dev_max", C.c_double), ("ex_abs_max", C.c_double)]
+
+    def asdict(self):
+        return {"t": self.t, "step": self.step, "psurv_nu": self.psurv_nu,
+                "psurv_nubar": self.psurv_nubar, "dP_max": self.dP_max, "dP_avg": self.dP_avg,
+                "M0": list(self.M0), "dM0": list(self.dM0),
+                "trace_dev_max": self.trace_dev_max, "ex_abs_max": self.ex_abs_max}
+
+
+_lib = None
+
+
+def load():
+    """Load libcosenu_b200.so (built in-tree by `python -m paper_2203_12866_b200.build`)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError("cosenu-b200: %s is missing; run `python -m paper_2203_12866_b200.build` "
+                           "(there is no CPU fallback)" % LIB_PATH)
+    L = C.CDLL(LIB_PATH)
+    dp = C.POINTER(C.c_double)
+    L.cosenu_create.restype = C.c_void_p
+    L.cosenu_create.argtypes = [C.c_int64, C.c_int32] + [C.c_double] * 5 + [C.c_int]
+    L.cosenu_workspace_bytes.restype = C.c_size_t
+    L.cosenu_workspace_bytes.argtypes = [C.c_void_p]
+    L.cosenu_attach.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
+    L.cosenu_set_option.argtypes = [C.c_void_p, C.c_int, C.c_double]
+    L.cosenu_init.argtypes = [C.c_void_p, C.c_uint64, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int]
+    L.cosenu_set_state.argtypes = [C.c_void_p, C.c_void_p, C.c_double]
+    L.cosenu_step.argtypes = [C.c_void_p, C.c_int64]
+    L.cosenu_get_state.argtypes = [C.c_void_p, C.c_void_p]
+    L.cosenu_get_moments.argtypes = [C.c_void_p, dp]
+    L.cosenu_diagnostics.argtypes = [C.c_void_p, C.POINTER(Diag)]
+    L.cosenu_sync.argtypes = [C.c_void_p]
+    L.cosenu_launch_count.restype = C.c_int64
+    L.cosenu_launch_count.argtypes = [C.c_void_p]
+    L.cosenu_stage_times.argtypes = [C.c_void_p, dp, C.POINTER(C.c_int64)]
+    L.cosenu_destroy.restype = None
+    L.cosenu_destroy.argtypes = [C.c_void_p]
+    L.cosenu_last_error.restype = C.c_char_p
+    L.cosenu_last_error.argtypes = [C.c_void_p]
+    _lib = L
+    return L
+
+
+class CosenuError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("cosenu error %d: %s" % (code, msg))
+        self.code = code
+
+
+class Cosenu:
+    """One solver handle on the current CUDA device.  Method names mirror the C ABI."""
+
+    def __init__(self, nz, nv, L, dt, omega, theta, mu, scheme, eps_ko=None, weno_eps=None, advect=True,
+                 lean_acc=False, use_torch_workspace=True, stream=None):
+        self._L = load()
+        self.nz, self.nv = int(nz), int(nv)
+        self.h = self._L.cosenu_create(nz, nv, L, dt, omega, theta, mu, scheme)
+        if not self.h:
+            raise CosenuError(EINVAL, self._L.cosenu_last_error(None).decode())
+        self._ws = None
+        if use_torch_workspace:
+            import torch
+            nbytes = self._L.cosenu_workspace_bytes(self.h)
+            # torch owns the device memory and the stream; the library only uses them
+            self._ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+            st = stream if stream is not None else torch.cuda.current_stream()
+            self._chk(self._L.cosenu_attach(self.h, self._ws.data_ptr(), nbytes, st.cuda_stream))
+        if eps_ko is not None:
+            self.set_option(OPT_EPS_KO, eps_ko)
+        if weno_eps is not None:
+            self.set_option(OPT_WENO_EPS, weno_eps)
+        if not advect:
+            self.set_option(OPT_ADVECT, 0)
+        if lean_acc:
+            self.set_option(OPT_LEAN_ACC, 1)
+
+    def _chk(self, rc):
+        if rc != 0:
+            raise CosenuError(rc, self._L.cosenu_last_error(self.h).decode())
+
+    def workspace_bytes(self):
+        return self._L.cosenu_workspace_bytes(self.h)
+
+    def set_option(self, key, value):
+        self._chk(self._L.cosenu_set_option(self.h, key, float(value)))
+
+    def init(self, seed, sigma_nu=0.6, sigma_nubar=0.5, alpha=0.9, pert_amp=1e-6, pert_kind=0):
+        self._chk(self._L.cosenu_init(self.h, seed, sigma_nu, sigma_nubar, alpha, pert_amp, pert_kind))
+
+    def set_state(self, state, t=0.0):
+        """state: numpy (8, nz, nv) float64, or a host torch tensor (pinned or not) of that shape."""
+        if isinstance(state, np.ndarray):
+            a = np.ascontiguousarray(state, dtype=np.float64)
+            assert a.shape == (8, self.nz, self.nv)
+            self._chk(self._L.cosenu_set_state(self.h, a.ctypes.data, t))
+        else:
+            assert tuple(state.shape) == (8, self.nz, self.nv) and state.is_contiguous() and not state.is_cuda
+            self._chk(self._L.cosenu_set_state(self.h, state.data_ptr(), t))
+
+    def step(self, n=1):
+        self._chk(self._L.cosenu_step(self.h, n))
+
+    def sync(self):
+        self._chk(self._L.cosenu_sync(self.h))
+
+    def get_state(self, out=None):
+        if out is None:
+            out = np.empty((8, self.nz, self.nv), dtype=np.float64)
+        if isinstance(out, np.ndarray):
+            assert out.shape == (8, self.nz, self.nv) and out.flags.c_contiguous and out.dtype == np.float64
+            self._chk(self._L.cosenu_get_state(self.h, out.ctypes.data))
+        else:
+            assert tuple(out.shape) == (8, self.nz, self.nv) and out.is_contiguous() and not out.is_cuda
+            self._chk(self._L.cosenu_get_state(self.h, out.data_ptr()))
+        return out
+
+    def get_moments(self):
+        out = np.empty((6, self.nz), dtype=np.float64)
+        self._chk(self._L.cosenu_get_moments(self.h, out.ctypes.data_as(C.POINTER(C.c_double))))
+        return out
+
+    def diagnostics(self):
+        d = Diag()
+        self._chk(self._L.cosenu_diagnostics(self.h, C.byref(d)))
+        return d.asdict()
+
+    def launch_count(self):
+        return self._L.cosenu_launch_count(self.h)
+
+    def stage_times(self):
+        ms = (C.c_double * 4)()
+        n = C.c_int64(0)
+        self._chk(self._L.cosenu_stage_times(self.h, ms, C.byref(n)))
+        return list(ms), n.value
+
+    def close(self):
+        if getattr(self, "h", None):
+            self._L.cosenu_destroy(self.h)
+            self.h = None
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

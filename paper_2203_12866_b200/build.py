@@ -1,0 +1,42 @@
+"""Build the CUDA library of cosenu-b200 in-tree for sm_100a.
+
+    python -m paper_2203_12866_b200.build [--force] [--verbose]
+        -> paper_2203_12866_b200/libcosenu_b200.so     (the product: kernels + C ABI, include/cosenu.h)
+        -> paper_2203_12866_b200/libcosenu_probe.so    (host build of csrc/weno7_math.h for the CPU tests)
+
+nvcc cross-compiles without a GPU.  -lineinfo keeps the ncu source page mapped to csrc/.
+"""
+import os
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+ROOT = os.path.dirname(HERE)
+LIB = os.path.join(HERE, "libcosenu_b200.so")
+PROBE = os.path.join(HERE, "libcosenu_probe.so")
+
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+              "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
+
+
+def _newer(out, deps):
+    return os.path.exists(out) and all(os.path.getmtime(out) >= os.path.getmtime(d) for d in deps)
+
+
+def build(force=False, verbose=False):
+    srcs = [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC))]
+    deps = srcs + [os.path.join(ROOT, "include", "cosenu.h"), os.path.abspath(__file__)]
+    if force or not _newer(LIB, deps):
+        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+              ["-o", LIB, os.path.join(CSRC, "cosenu_api.cu")]
+        subprocess.run(cmd, check=True)
+    if force or not _newer(PROBE, deps):
+        subprocess.run(["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-fPIC", "-shared", "-o", PROBE,
+                        os.path.join(CSRC, "host_probe.cpp")], check=True)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

@@ -1,0 +1,130 @@
+// aux_kernels.cuh -- kernels off the timed path: ghost rows, the moments of a freshly uploaded state,
+// and the diagnostics reductions.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace cosenu_dev {
+
+// periodic ghost rows of one state buffer: rows -G..-1 <- nz-G..nz-1, rows nz..nz+G-1 <- 0..G-1
+__global__ void fill_ghosts_kernel(double* y, long long nz, int nvp, long long comp_stride, int g) {
+  const long long n = (long long)8 * 2 * g * nvp;
+  for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < n; q += (long long)gridDim.x * blockDim.x) {
+    const int j = (int)(q % nvp);
+    const int r = (int)((q / nvp) % (2 * g));
+    const int c = (int)(q / ((long long)nvp * 2 * g));
+    double* base = y + c * comp_stride;
+    if (r < g) base[(long long)r * nvp + j] = base[(nz + r) * nvp + j];                  // device row r <- z = nz-g+r
+    else base[(nz + r) * nvp + j] = base[(long long)r * nvp + j];                        // device row nz+r <- z = r-g
+  }
+}
+
+// the 6 velocity moments per z of a state (S1; Riemann sum of PAPER.md:78): one warp per z row,
+// lanes stride over v, fixed shuffle tree => reproducible.  mom[6][nz], already times dv.
+__global__ void moments_kernel(const double* __restrict__ y, double* __restrict__ mom, long long nz, int nv, int nvp,
+                               long long comp_stride, int g, double dv) {
+  const int warps = blockDim.x / 32, wid = threadIdx.x / 32, lane = threadIdx.x % 32;
+  for (long long iz = blockIdx.x * (long long)warps + wid; iz < nz; iz += (long long)gridDim.x * warps) {
+    double m[6] = {0, 0, 0, 0, 0, 0};
+    const double* row = y + (iz + g) * nvp;
+    for (int j = lane; j < nv; j += 32) {
+      const double v = __dadd_rn(-1.0, __dmul_rn((double)j + 0.5, dv));
+      const double dd = (row[j] - row[comp_stride + j]) - (row[4 * comp_stride + j] - row[5 * comp_stride + j]);
+      const double dr = row[2 * comp_stride + j] - row[6 * comp_stride + j];
+      const double di = row[3 * comp_stride + j] + row[7 * comp_stride + j];
+      m[0] += dd; m[1] = fma(v, dd, m[1]);
+      m[2] += dr; m[3] = fma(v, dr, m[3]);
+      m[4] += di; m[5] = fma(v, di, m[5]);
+    }
+#pragma unroll
+    for (int q = 0; q < 6; ++q) {
+#pragma unroll
+      for (int off = 16; off > 0; off >>= 1) m[q] += __shfl_xor_sync(0xffffffffu, m[q], off);
+      if (lane == 0) mom[(long long)q * nz + iz] = m[q] * dv;
+    }
+  }
+}
+
+__device__ __forceinline__ double plen(double ee, double xx, double r, double i) {
+  const double d = ee - xx;
+  return sqrt(fma(d, d, 4.0 * fma(r, r, i * i)));  // |P| of Eq. (4), un-normalised
+}
+
+// z-slab partial sums of |P|(z,v) and P0(z,v) per species: part[b][4][nv] (|P|_nu, P0_nu, |P|_nubar, P0_nubar)
+__global__ void diag_ref_kernel(const double* __restrict__ y, double* __restrict__ part, long long nz, int nv, int nvp,
+                                long long comp_stride, int g) {
+  const long long rows_per = (nz + gridDim.x - 1) / gridDim.x;
+  const long long z0 = blockIdx.x * rows_per, z1 = min(nz, z0 + rows_per);
+  for (int j = threadIdx.x; j < nv; j += blockDim.x) {
+    double a[4] = {0, 0, 0, 0};
+    for (long long iz = z0; iz < z1; ++iz) {
+      const double* q = y + (iz + g) * nvp + j;
+#pragma unroll
+      for (int s = 0; s < 2; ++s) {
+        const double ee = q[(4 * s) * comp_stride], xx = q[(4 * s + 1) * comp_stride];
+        a[2 * s] += plen(ee, xx, q[(4 * s + 2) * comp_stride], q[(4 * s + 3) * comp_stride]);
+        a[2 * s + 1] += ee + xx;
+      }
+    }
+#pragma unroll
+    for (int m = 0; m < 4; ++m) part[((long long)blockIdx.x * 4 + m) * nv + j] = a[m];
+  }
+}
+
+constexpr int DIAG_NSUM = 7;  // see_nu, see_nubar, sum| |P_nu| - Pref |, M0x, M0y, M0z, (spare)
+constexpr int DIAG_NMAX = 3;  // dP_max, trace_dev_max, ex_abs_max
+constexpr int DIAG_NVAL = DIAG_NSUM + DIAG_NMAX;
+
+// per-block partial diagnostics over a z-slab: part[b][DIAG_NVAL]
+__global__ void diag_kernel(const double* __restrict__ y, const double* __restrict__ pref /*[2][nv]*/,
+                            const double* __restrict__ p0ref /*[2][nv]*/, double* __restrict__ part, long long nz,
+                            int nv, int nvp, long long comp_stride, int g) {
+  const long long rows_per = (nz + gridDim.x - 1) / gridDim.x;
+  const long long z0 = blockIdx.x * rows_per, z1 = min(nz, z0 + rows_per);
+  double sm[DIAG_NSUM] = {0, 0, 0, 0, 0, 0, 0};
+  double mx[DIAG_NMAX] = {0, 0, 0};
+  for (int j = threadIdx.x; j < nv; j += blockDim.x) {
+    const double pr[2] = {pref[j], pref[nv + j]}, p0[2] = {p0ref[j], p0ref[nv + j]};
+    for (long long iz = z0; iz < z1; ++iz) {
+      const double* q = y + (iz + g) * nvp + j;
+      double c[8];
+#pragma unroll
+      for (int k = 0; k < 8; ++k) c[k] = q[k * comp_stride];
+#pragma unroll
+      for (int s = 0; s < 2; ++s) {
+        const double ee = c[4 * s], xx = c[4 * s + 1], r = c[4 * s + 2], im = c[4 * s + 3];
+        sm[s] += ee;
+        const double P = plen(ee, xx, r, im);
+        if (pr[s] > 0) mx[0] = fmax(mx[0], fabs(P / pr[s] - 1.0));   // Eq. (22)
+        if (s == 0) sm[2] += fabs(P - pr[0]);                        // numerator of Eq. (23)
+        mx[1] = fmax(mx[1], fabs(ee + xx - p0[s]));
+        mx[2] = fmax(mx[2], sqrt(fma(r, r, im * im)));
+      }
+      // Eq. (19) in stored variables: P = (2 Re, -2 Im, ee - xx) of D = rho - rhobar^*
+      sm[3] += 2.0 * (c[2] - c[6]);
+      sm[4] += -2.0 * (c[3] + c[7]);
+      sm[5] += (c[0] - c[1]) - (c[4] - c[5]);
+    }
+  }
+  __shared__ double red[32][DIAG_NVAL];
+  const int lane = threadIdx.x % 32, wid = threadIdx.x / 32, nw = blockDim.x / 32;
+#pragma unroll
+  for (int k = 0; k < DIAG_NSUM; ++k)
+    for (int off = 16; off > 0; off >>= 1) sm[k] += __shfl_xor_sync(0xffffffffu, sm[k], off);
+#pragma unroll
+  for (int k = 0; k < DIAG_NMAX; ++k)
+    for (int off = 16; off > 0; off >>= 1) mx[k] = fmax(mx[k], __shfl_xor_sync(0xffffffffu, mx[k], off));
+  if (lane == 0) {
+    for (int k = 0; k < DIAG_NSUM; ++k) red[wid][k] = sm[k];
+    for (int k = 0; k < DIAG_NMAX; ++k) red[wid][DIAG_NSUM + k] = mx[k];
+  }
+  __syncthreads();
+  if (threadIdx.x < DIAG_NVAL) {
+    const int k = threadIdx.x;
+    double a = red[0][k];
+    for (int w = 1; w < nw; ++w) a = k < DIAG_NSUM ? a + red[w][k] : fmax(a, red[w][k]);
+    part[(long long)blockIdx.x * DIAG_NVAL + k] = a;
+  }
+}
+
+}  // namespace cosenu_dev

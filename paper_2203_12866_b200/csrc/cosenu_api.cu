@@ -1,0 +1,536 @@
+// cosenu_api.cu -- the C ABI of include/cosenu.h: handle, workspace, TMA descriptors, launches.
+// Host logic only; every step of the path runs in the kernels of stage_kernels.cuh / aux_kernels.cuh.
+#include "../../include/cosenu.h"
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "aux_kernels.cuh"
+#include "stage_kernels.cuh"
+
+using namespace cosenu_dev;
+
+namespace {
+
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// tile shapes: TZ rows per CTA, NSEG z-segments, VC beams per chunk
+constexpr int FD_TZ = 32, FD_NSEG = 8;
+constexpr int WN_TZ = 32, WN_NSEG = 8;
+constexpr int DIAG_BLOCKS = 592, DIAG_THREADS = 256, REF_BLOCKS = 148;
+
+std::string g_create_err;
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+}  // namespace
+
+struct cosenu {
+  int64_t nz; int32_t nv; int nvp;
+  double L, dt, omega, theta, mu; int scheme;
+  double eps_ko = 0.1, weno_eps = 1e-6;
+  int advect = 1, lean_acc = 0, stage_timing = 0;
+  double dz, dv;
+  int device = 0;
+  int vc = 32, tz = 32;  // chunk width, rows per CTA
+
+  // workspace
+  void* ws = nullptr; size_t ws_bytes = 0; bool ws_owned = false;
+  cudaStream_t stream = nullptr;
+  double *U = nullptr, *Y1 = nullptr, *Y2 = nullptr, *ACC = nullptr;
+  double* M[2] = {nullptr, nullptr};
+  double *d_pref = nullptr, *d_p0ref = nullptr, *d_refpart = nullptr, *d_diagpart = nullptr;
+  int64_t comp_stride = 0; size_t state_elems = 0;
+  int mcur = 0;  // M[mcur] holds the moments of U
+  CUtensorMap tm_U, tm_Y1, tm_Y2;
+  bool maps_ready = false;
+
+  bool have_state = false;
+  double t = 0; int64_t step = 0;
+  int64_t launches = 0;
+  double sum_ee0[2] = {0, 0}, M0_init[3] = {0, 0, 0}, pref_sum_nu = 0;
+
+  // stage timing
+  std::vector<cudaEvent_t> ev_pool; size_t ev_used = 0;
+  double stage_ms[4] = {0, 0, 0, 0}; int64_t stage_n = 0;
+
+  std::string err;
+};
+
+namespace {
+
+int fail(cosenu* h, int code, const std::string& msg) {
+  if (h) h->err = msg; else g_create_err = msg;
+  return code;
+}
+int cuda_fail(cosenu* h, cudaError_t e, const char* what) {
+  return fail(h, COSENU_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define CK(call)                                                  \
+  do {                                                            \
+    cudaError_t e_ = (call);                                      \
+    if (e_ != cudaSuccess) return cuda_fail(h, e_, #call);        \
+  } while (0)
+
+size_t workspace_layout(const cosenu* h, size_t off[10]) {
+  const size_t st = align_up(sizeof(double) * 8 * (size_t)(h->nz + 2 * G) * h->nvp, 256);
+  const size_t mo = align_up(sizeof(double) * 6 * (size_t)h->nz, 256);
+  const size_t rf = align_up(sizeof(double) * 2 * (size_t)h->nv, 256);
+  const size_t rp = align_up(sizeof(double) * REF_BLOCKS * 4 * (size_t)h->nv, 256);
+  const size_t dp = align_up(sizeof(double) * DIAG_BLOCKS * DIAG_NVAL, 256);
+  size_t o = 0;
+  off[0] = o; o += st;  // U
+  off[1] = o; o += st;  // Y1
+  off[2] = o; o += st;  // Y2
+  off[3] = o; o += st;  // ACC
+  off[4] = o; o += mo;  // M[0]
+  off[5] = o; o += mo;  // M[1]
+  off[6] = o; o += rf;  // pref
+  off[7] = o; o += rf;  // p0ref
+  off[8] = o; o += rp;  // ref partials
+  off[9] = o; o += dp;  // diag partials
+  return o;
+}
+
+int make_map(cosenu* h, PFN_encodeTiled enc, CUtensorMap* map, double* base, int rows_box) {
+  const cuuint64_t gdim[3] = {(cuuint64_t)h->nv, (cuuint64_t)(h->nz + 2 * G), 8};
+  const cuuint64_t gstr[2] = {(cuuint64_t)h->nvp * 8, (cuuint64_t)h->comp_stride * 8};
+  const cuuint32_t box[3] = {(cuuint32_t)h->vc, (cuuint32_t)rows_box, 8};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, base, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                   CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(h, COSENU_ECUDA, "cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")");
+  return COSENU_OK;
+}
+
+int ensure_workspace(cosenu* h) {
+  if (h->maps_ready) return COSENU_OK;
+  CK(cudaSetDevice(h->device));
+  size_t off[10];
+  const size_t need = workspace_layout(h, off);
+  if (!h->ws) {
+    cudaError_t e = cudaMalloc(&h->ws, need);
+    if (e != cudaSuccess) { h->ws = nullptr; return fail(h, e == cudaErrorMemoryAllocation ? COSENU_ENOMEM : COSENU_ECUDA,
+                                                        std::string("cudaMalloc workspace: ") + cudaGetErrorString(e)); }
+    h->ws_bytes = need; h->ws_owned = true;
+  }
+  char* b = static_cast<char*>(h->ws);
+  h->U = (double*)(b + off[0]); h->Y1 = (double*)(b + off[1]); h->Y2 = (double*)(b + off[2]); h->ACC = (double*)(b + off[3]);
+  h->M[0] = (double*)(b + off[4]); h->M[1] = (double*)(b + off[5]);
+  h->d_pref = (double*)(b + off[6]); h->d_p0ref = (double*)(b + off[7]);
+  h->d_refpart = (double*)(b + off[8]); h->d_diagpart = (double*)(b + off[9]);
+  CK(cudaMemsetAsync(h->ws, 0, need, h->stream));
+
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qr;
+  CK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr));
+  if (!fn || qr != cudaDriverEntryPointSuccess) return fail(h, COSENU_ECUDA, "cuTensorMapEncodeTiled not available in this driver");
+  PFN_encodeTiled enc = reinterpret_cast<PFN_encodeTiled>(fn);
+  const int rows = h->tz + 2 * (h->scheme == COSENU_FD4_KO3 ? 2 : 4);
+  int rc;
+  if ((rc = make_map(h, enc, &h->tm_U, h->U, rows))) return rc;
+  if ((rc = make_map(h, enc, &h->tm_Y1, h->Y1, rows))) return rc;
+  if ((rc = make_map(h, enc, &h->tm_Y2, h->Y2, rows))) return rc;
+  h->maps_ready = true;
+  return COSENU_OK;
+}
+
+template <int SCHEME, int KIND, int TZ, int NSEG, int VC>
+int launch_one(cosenu* h, const CUtensorMap& map, const StageParams& p) {
+  auto kern = stage_kernel<SCHEME, KIND, TZ, NSEG, VC>;
+  constexpr size_t smem = StageSmem<SCHEME, TZ, VC>::bytes;
+  static bool configured = false;  // per instantiation; attributes are per-function and per-context
+  if (!configured) {
+    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    configured = true;
+  }
+  const unsigned grid = (unsigned)((h->nz + TZ - 1) / TZ);
+  kern<<<grid, NSEG * VC, smem, h->stream>>>(map, p);
+  CK(cudaGetLastError());
+  h->launches++;
+  return COSENU_OK;
+}
+
+template <int SCHEME, int TZ, int NSEG, int VC>
+int launch_kind(cosenu* h, int kind, const CUtensorMap& map, const StageParams& p) {
+  switch (kind) {
+    case FIRST: return launch_one<SCHEME, FIRST, TZ, NSEG, VC>(h, map, p);
+    case FIRST_LEAN: return launch_one<SCHEME, FIRST_LEAN, TZ, NSEG, VC>(h, map, p);
+    case MID: return launch_one<SCHEME, MID, TZ, NSEG, VC>(h, map, p);
+    case MID_REBUILD: return launch_one<SCHEME, MID_REBUILD, TZ, NSEG, VC>(h, map, p);
+    default: return launch_one<SCHEME, LAST, TZ, NSEG, VC>(h, map, p);
+  }
+}
+
+int launch_stage(cosenu* h, int kind, const CUtensorMap& map, const StageParams& p) {
+  if (h->scheme == COSENU_FD4_KO3) {
+    if (h->vc == 16) return launch_kind<0, FD_TZ, 2 * FD_NSEG, 16>(h, kind, map, p);
+    return launch_kind<0, FD_TZ, FD_NSEG, 32>(h, kind, map, p);
+  }
+  if (h->vc == 16) return launch_kind<1, WN_TZ, 2 * WN_NSEG, 16>(h, kind, map, p);
+  return launch_kind<1, WN_TZ, WN_NSEG, 32>(h, kind, map, p);
+}
+
+StageParams base_params(const cosenu* h) {
+  StageParams p;
+  std::memset(&p, 0, sizeof(p));
+  p.nz = h->nz; p.nv = h->nv; p.nvp = h->nvp; p.comp_stride = h->comp_stride;
+  p.mu = h->mu;
+  p.A0 = -h->omega * std::cos(2.0 * h->theta);
+  p.Br0 = 0.5 * h->omega * std::sin(2.0 * h->theta);
+  p.dv = h->dv;
+  const double sw = h->advect ? 1.0 : 0.0;
+  p.cadv = sw * (-1.0 / (12.0 * h->dz));
+  p.cko = sw * (-h->eps_ko / (16.0 * h->dz));
+  p.ninv_dz = sw * (-1.0 / h->dz);
+  p.weno_eps = h->weno_eps;
+  return p;
+}
+
+cudaEvent_t next_event(cosenu* h) {
+  if (h->ev_used == h->ev_pool.size()) {
+    cudaEvent_t e = nullptr;
+    if (cudaEventCreate(&e) != cudaSuccess) return nullptr;
+    h->ev_pool.push_back(e);
+  }
+  return h->ev_pool[h->ev_used++];
+}
+
+int drain_events(cosenu* h) {
+  if (h->ev_used == 0) return COSENU_OK;
+  CK(cudaStreamSynchronize(h->stream));
+  for (size_t s = 0; s + 5 <= h->ev_used; s += 5) {
+    for (int k = 0; k < 4; ++k) {
+      float ms = 0;
+      CK(cudaEventElapsedTime(&ms, h->ev_pool[s + k], h->ev_pool[s + k + 1]));
+      h->stage_ms[k] += ms;
+    }
+    h->stage_n++;
+  }
+  h->ev_used = 0;
+  return COSENU_OK;
+}
+
+// one classical RK4 step = 4 fused stage launches.  Buffers: U -> Y1 -> Y2 -> Y1 -> U, accumulator ACC.
+int one_step(cosenu* h) {
+  const double dt = h->dt;
+  StageParams p = base_params(h);
+  const bool tm = h->stage_timing != 0;
+  int rc;
+  cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+  if (tm) {
+    if (h->ev_used + 5 > 5 * 4096) { if ((rc = drain_events(h))) return rc; }
+    for (int k = 0; k < 5; ++k) if (!(ev[k] = next_event(h))) return fail(h, COSENU_ECUDA, "cudaEventCreate failed");
+    CK(cudaEventRecord(ev[0], h->stream));
+  }
+  double* Min = h->M[h->mcur];
+  double* Mout = h->M[h->mcur ^ 1];
+  // stage 1: k1 = RHS(U); Y1 = U + dt/2 k1; ACC = U + dt/6 k1
+  p.u0 = nullptr; p.acc_in = nullptr; p.y_out = h->Y1; p.acc_out = h->ACC; p.mom_in = Min; p.mom_out = Mout;
+  p.cy = 0.5 * dt; p.ca = dt / 6.0;
+  if ((rc = launch_stage(h, h->lean_acc ? FIRST_LEAN : FIRST, h->tm_U, p))) return rc;
+  if (tm) CK(cudaEventRecord(ev[1], h->stream));
+  // stage 2: k2 = RHS(Y1); Y2 = U + dt/2 k2; ACC += dt/3 k2
+  p.u0 = h->U; p.acc_in = h->ACC; p.y_out = h->Y2; p.acc_out = h->ACC; p.mom_in = Mout; p.mom_out = Min;
+  p.cy = 0.5 * dt; p.ca = dt / 3.0;
+  if ((rc = launch_stage(h, h->lean_acc ? MID_REBUILD : MID, h->tm_Y1, p))) return rc;
+  if (tm) CK(cudaEventRecord(ev[2], h->stream));
+  // stage 3: k3 = RHS(Y2); Y1 = U + dt k3; ACC += dt/3 k3
+  p.y_out = h->Y1; p.mom_in = Min; p.mom_out = Mout;
+  p.cy = dt; p.ca = dt / 3.0;
+  if ((rc = launch_stage(h, MID, h->tm_Y2, p))) return rc;
+  if (tm) CK(cudaEventRecord(ev[3], h->stream));
+  // stage 4: k4 = RHS(Y1); U = ACC + dt/6 k4
+  p.u0 = nullptr; p.y_out = h->U; p.acc_out = nullptr; p.mom_in = Mout; p.mom_out = Min;
+  p.cy = dt / 6.0; p.ca = 0.0;
+  if ((rc = launch_stage(h, LAST, h->tm_Y1, p))) return rc;
+  if (tm) CK(cudaEventRecord(ev[4], h->stream));
+  // moments of the new U are in Min = M[mcur] again
+  h->t += dt; h->step += 1;
+  return COSENU_OK;
+}
+
+int run_diag(cosenu* h, double sums[DIAG_NSUM], double maxs[DIAG_NMAX]) {
+  diag_kernel<<<DIAG_BLOCKS, DIAG_THREADS, 0, h->stream>>>(h->U, h->d_pref, h->d_p0ref, h->d_diagpart, h->nz, h->nv,
+                                                           h->nvp, h->comp_stride, G);
+  CK(cudaGetLastError());
+  h->launches++;
+  std::vector<double> part((size_t)DIAG_BLOCKS * DIAG_NVAL);
+  CK(cudaMemcpyAsync(part.data(), h->d_diagpart, sizeof(double) * part.size(), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  long double s[DIAG_NSUM];
+  for (int k = 0; k < DIAG_NSUM; ++k) s[k] = 0;
+  for (int k = 0; k < DIAG_NMAX; ++k) maxs[k] = 0;
+  for (int b = 0; b < DIAG_BLOCKS; ++b) {
+    for (int k = 0; k < DIAG_NSUM; ++k) s[k] += part[(size_t)b * DIAG_NVAL + k];
+    for (int k = 0; k < DIAG_NMAX; ++k) maxs[k] = std::fmax(maxs[k], part[(size_t)b * DIAG_NVAL + DIAG_NSUM + k]);
+  }
+  for (int k = 0; k < DIAG_NSUM; ++k) sums[k] = (double)s[k];
+  return COSENU_OK;
+}
+
+// after U has been uploaded: ghosts, moments, diagnostic references
+int finish_upload(cosenu* h, double t) {
+  fill_ghosts_kernel<<<64, 256, 0, h->stream>>>(h->U, h->nz, h->nvp, h->comp_stride, G);
+  CK(cudaGetLastError());
+  h->mcur = 0;
+  moments_kernel<<<592, 256, 0, h->stream>>>(h->U, h->M[0], h->nz, h->nv, h->nvp, h->comp_stride, G, h->dv);
+  CK(cudaGetLastError());
+  diag_ref_kernel<<<REF_BLOCKS, 256, 0, h->stream>>>(h->U, h->d_refpart, h->nz, h->nv, h->nvp, h->comp_stride, G);
+  CK(cudaGetLastError());
+  h->launches += 3;
+  std::vector<double> part((size_t)REF_BLOCKS * 4 * h->nv);
+  CK(cudaMemcpyAsync(part.data(), h->d_refpart, sizeof(double) * part.size(), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  std::vector<double> pref(2 * (size_t)h->nv), p0ref(2 * (size_t)h->nv);
+  long double prsum = 0;
+  for (int j = 0; j < h->nv; ++j) {
+    long double a[4] = {0, 0, 0, 0};
+    for (int b = 0; b < REF_BLOCKS; ++b)
+      for (int m = 0; m < 4; ++m) a[m] += part[((size_t)b * 4 + m) * h->nv + j];
+    pref[j] = (double)(a[0] / h->nz); p0ref[j] = (double)(a[1] / h->nz);
+    pref[h->nv + j] = (double)(a[2] / h->nz); p0ref[h->nv + j] = (double)(a[3] / h->nz);
+    prsum += pref[j];
+  }
+  h->pref_sum_nu = (double)(prsum * h->nz);
+  CK(cudaMemcpyAsync(h->d_pref, pref.data(), sizeof(double) * pref.size(), cudaMemcpyHostToDevice, h->stream));
+  CK(cudaMemcpyAsync(h->d_p0ref, p0ref.data(), sizeof(double) * p0ref.size(), cudaMemcpyHostToDevice, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  double sums[DIAG_NSUM], maxs[DIAG_NMAX];
+  int rc = run_diag(h, sums, maxs);
+  if (rc) return rc;
+  h->sum_ee0[0] = sums[0]; h->sum_ee0[1] = sums[1];
+  for (int m = 0; m < 3; ++m) h->M0_init[m] = sums[3 + m] * (h->dz * h->dv);
+  h->t = t; h->step = 0; h->have_state = true;
+  return COSENU_OK;
+}
+
+inline uint64_t splitmix64_next(uint64_t& s) {
+  uint64_t z = (s += 0x9E3779B97F4A7C15ull);
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  return z ^ (z >> 31);
+}
+
+}  // namespace
+
+// ================================================================================ C ABI
+extern "C" cosenu_t* cosenu_create(int64_t nz, int32_t nv, double L, double dt, double omega, double theta, double mu,
+                                   int scheme) {
+  if (nz < 16 || nz > 2000000000ll || nv < 2 || nv > (1 << 20) || !(L > 0) || !(dt > 0) || (scheme != 0 && scheme != 1) ||
+      !std::isfinite(L) || !std::isfinite(dt) || !std::isfinite(omega) || !std::isfinite(theta) || !std::isfinite(mu)) {
+    g_create_err = "cosenu_create: invalid argument";
+    return nullptr;
+  }
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) { g_create_err = std::string("cosenu_create: no CUDA device: ") + cudaGetErrorString(e); return nullptr; }
+  cudaDeviceProp prop;
+  e = cudaGetDeviceProperties(&prop, dev);
+  if (e != cudaSuccess) { g_create_err = std::string("cosenu_create: ") + cudaGetErrorString(e); return nullptr; }
+  if (prop.major != 10) {
+    g_create_err = "cosenu_create: this library holds sm_100a code only; device is sm_" + std::to_string(prop.major) +
+                   std::to_string(prop.minor);
+    return nullptr;
+  }
+  cosenu* h = new (std::nothrow) cosenu();
+  if (!h) { g_create_err = "out of memory"; return nullptr; }
+  h->nz = nz; h->nv = nv; h->L = L; h->dt = dt; h->omega = omega; h->theta = theta; h->mu = mu; h->scheme = scheme;
+  h->device = dev;
+  h->nvp = (nv + 3) / 4 * 4;
+  h->dz = L / (double)nz; h->dv = 2.0 / (double)nv;
+  h->comp_stride = (int64_t)(nz + 2 * G) * h->nvp;
+  h->vc = nv <= 16 ? 16 : 32;
+  h->tz = scheme == COSENU_FD4_KO3 ? FD_TZ : WN_TZ;
+  return h;
+}
+
+extern "C" size_t cosenu_workspace_bytes(const cosenu_t* h) {
+  if (!h) return 0;
+  size_t off[10];
+  return workspace_layout(h, off);
+}
+
+extern "C" int cosenu_attach(cosenu_t* h, void* dev_workspace, size_t bytes, void* cuda_stream) {
+  if (!h) return COSENU_EINVAL;
+  if (h->maps_ready) return fail(h, COSENU_ESTATE, "cosenu_attach: workspace already in use");
+  if (dev_workspace) {
+    if (bytes < cosenu_workspace_bytes(h) || (reinterpret_cast<uintptr_t>(dev_workspace) & 255))
+      return fail(h, COSENU_EINVAL, "cosenu_attach: workspace too small or not 256-byte aligned");
+    h->ws = dev_workspace; h->ws_bytes = bytes; h->ws_owned = false;
+  }
+  h->stream = static_cast<cudaStream_t>(cuda_stream);
+  return COSENU_OK;
+}
+
+extern "C" int cosenu_set_option(cosenu_t* h, int key, double value) {
+  if (!h) return COSENU_EINVAL;
+  switch (key) {
+    case COSENU_OPT_EPS_KO: if (!(value >= 0) || !std::isfinite(value)) break; h->eps_ko = value; return COSENU_OK;
+    case COSENU_OPT_WENO_EPS: if (!(value > 0) || !(value <= 1e30)) break; h->weno_eps = value; return COSENU_OK;
+    case COSENU_OPT_ADVECT: h->advect = value != 0; return COSENU_OK;
+    case COSENU_OPT_LEAN_ACC: h->lean_acc = value != 0; return COSENU_OK;
+    case COSENU_OPT_STAGE_TIMING: {
+      int rc = drain_events(h);
+      if (rc) return rc;
+      h->stage_timing = value != 0;
+      for (int k = 0; k < 4; ++k) h->stage_ms[k] = 0;
+      h->stage_n = 0;
+      return COSENU_OK;
+    }
+  }
+  return fail(h, COSENU_EINVAL, "cosenu_set_option: bad key or value");
+}
+
+extern "C" int cosenu_set_state(cosenu_t* h, const double* host_state, double t) {
+  if (!h || !host_state || !std::isfinite(t)) return h ? fail(h, COSENU_EINVAL, "cosenu_set_state: invalid argument") : COSENU_EINVAL;
+  int rc = ensure_workspace(h);
+  if (rc) return rc;
+  for (int c = 0; c < 8; ++c) {
+    CK(cudaMemcpy2DAsync(h->U + c * h->comp_stride + (size_t)G * h->nvp, sizeof(double) * h->nvp,
+                         host_state + (size_t)c * h->nz * h->nv, sizeof(double) * h->nv, sizeof(double) * h->nv,
+                         (size_t)h->nz, cudaMemcpyHostToDevice, h->stream));
+  }
+  return finish_upload(h, t);
+}
+
+extern "C" int cosenu_init(cosenu_t* h, uint64_t seed, double sigma_nu, double sigma_nubar, double alpha, double pert_amp,
+                           int pert_kind) {
+  if (!h) return COSENU_EINVAL;
+  if (!(sigma_nu > 0) || !(sigma_nubar > 0) || !(alpha >= 0) || !std::isfinite(pert_amp) || pert_kind < 0 || pert_kind > 2)
+    return fail(h, COSENU_EINVAL, "cosenu_init: invalid argument");
+  const int nv = h->nv; const int64_t nz = h->nz;
+  std::vector<double> st;
+  try { st.assign(8 * (size_t)nz * nv, 0.0); } catch (...) { return fail(h, COSENU_ENOMEM, "cosenu_init: host out of memory"); }
+  // Eq. (20), normalised so that sum_j g_j dv = 1; g_bar carries alpha
+  std::vector<double> g(nv), gb(nv);
+  double sg = 0, sgb = 0;
+  for (int j = 0; j < nv; ++j) {
+    const double v = -1.0 + (j + 0.5) * h->dv;
+    g[j] = std::exp(-(v - 1.0) * (v - 1.0) / (2.0 * sigma_nu * sigma_nu));
+    gb[j] = std::exp(-(v - 1.0) * (v - 1.0) / (2.0 * sigma_nubar * sigma_nubar));
+    sg += g[j]; sgb += gb[j];
+  }
+  for (int j = 0; j < nv; ++j) { g[j] = g[j] / (sg * h->dv); gb[j] = alpha * (gb[j] / (sgb * h->dv)); }
+  const double two_pi = 6.283185307179586476925286766559;
+  std::vector<double> pr(nz), pi(nz), dd(nz, 1.0);
+  uint64_t s = seed;
+  if (pert_kind == 0) {
+    for (int64_t i = 0; i < nz; ++i) {
+      const double u = (double)(splitmix64_next(s) >> 11) * (1.0 / 9007199254740992.0);
+      pr[i] = pert_amp * std::cos(two_pi * u); pi[i] = pert_amp * std::sin(two_pi * u);
+    }
+  } else if (pert_kind == 1) {
+    const int K = 16; double ph[K];
+    for (int q = 0; q < K; ++q) ph[q] = two_pi * ((double)(splitmix64_next(s) >> 11) * (1.0 / 9007199254740992.0));
+    for (int64_t i = 0; i < nz; ++i) {
+      double a = 0, b = 0;
+      for (int q = 0; q < K; ++q) {
+        const double arg = two_pi * (double)(q + 1) * (double)i / (double)nz + ph[q];
+        a += std::cos(arg); b += std::sin(arg);
+      }
+      pr[i] = pert_amp * a / 4.0; pi[i] = pert_amp * b / 4.0;
+    }
+  } else {
+    for (int64_t i = 0; i < nz; ++i) {
+      const double zc = (h->scheme == COSENU_FV_WENO7 ? (i + 0.5) : (double)i) * h->dz - 0.5 * h->L;
+      const double e = pert_amp * std::exp(-zc * zc / 50.0);
+      pr[i] = 0.5 * e; pi[i] = 0.0; dd[i] = std::sqrt(1.0 - e * e);
+    }
+  }
+  const size_t pl = (size_t)nz * nv;
+  for (int64_t i = 0; i < nz; ++i)
+    for (int j = 0; j < nv; ++j) {
+      const size_t q = (size_t)i * nv + j;
+      st[0 * pl + q] = g[j] * 0.5 * (1.0 + dd[i]);  st[1 * pl + q] = g[j] * 0.5 * (1.0 - dd[i]);
+      st[2 * pl + q] = g[j] * pr[i];                st[3 * pl + q] = g[j] * pi[i];
+      st[4 * pl + q] = gb[j] * 0.5 * (1.0 + dd[i]); st[5 * pl + q] = gb[j] * 0.5 * (1.0 - dd[i]);
+      st[6 * pl + q] = gb[j] * pr[i];               st[7 * pl + q] = gb[j] * pi[i];
+    }
+  return cosenu_set_state(h, st.data(), 0.0);
+}
+
+extern "C" int cosenu_step(cosenu_t* h, int64_t n) {
+  if (!h || n < 0) return h ? fail(h, COSENU_EINVAL, "cosenu_step: n < 0") : COSENU_EINVAL;
+  if (!h->have_state) return fail(h, COSENU_ESTATE, "cosenu_step: no state, call cosenu_init or cosenu_set_state first");
+  CK(cudaSetDevice(h->device));
+  for (int64_t s = 0; s < n; ++s) {
+    int rc = one_step(h);
+    if (rc) return rc;
+  }
+  return COSENU_OK;
+}
+
+extern "C" int cosenu_sync(cosenu_t* h) {
+  if (!h) return COSENU_EINVAL;
+  CK(cudaStreamSynchronize(h->stream));
+  return COSENU_OK;
+}
+
+extern "C" int cosenu_get_state(cosenu_t* h, double* host_out) {
+  if (!h || !host_out) return COSENU_EINVAL;
+  if (!h->have_state) return fail(h, COSENU_ESTATE, "cosenu_get_state: no state");
+  for (int c = 0; c < 8; ++c) {
+    CK(cudaMemcpy2DAsync(host_out + (size_t)c * h->nz * h->nv, sizeof(double) * h->nv,
+                         h->U + c * h->comp_stride + (size_t)G * h->nvp, sizeof(double) * h->nvp, sizeof(double) * h->nv,
+                         (size_t)h->nz, cudaMemcpyDeviceToHost, h->stream));
+  }
+  CK(cudaStreamSynchronize(h->stream));
+  return COSENU_OK;
+}
+
+extern "C" int cosenu_get_moments(cosenu_t* h, double* host_out) {
+  if (!h || !host_out) return COSENU_EINVAL;
+  if (!h->have_state) return fail(h, COSENU_ESTATE, "cosenu_get_moments: no state");
+  CK(cudaMemcpyAsync(host_out, h->M[h->mcur], sizeof(double) * 6 * (size_t)h->nz, cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  return COSENU_OK;
+}
+
+extern "C" int cosenu_diagnostics(cosenu_t* h, cosenu_diag_t* d) {
+  if (!h || !d) return COSENU_EINVAL;
+  if (!h->have_state) return fail(h, COSENU_ESTATE, "cosenu_diagnostics: no state");
+  double sums[DIAG_NSUM], maxs[DIAG_NMAX];
+  int rc = run_diag(h, sums, maxs);
+  if (rc) return rc;
+  d->t = h->t; d->step = h->step;
+  d->psurv_nu = h->sum_ee0[0] != 0 ? sums[0] / h->sum_ee0[0] : 0.0;
+  d->psurv_nubar = h->sum_ee0[1] != 0 ? sums[1] / h->sum_ee0[1] : 0.0;
+  d->dP_max = maxs[0];
+  d->dP_avg = h->pref_sum_nu > 0 ? sums[2] / h->pref_sum_nu : 0.0;
+  for (int m = 0; m < 3; ++m) { d->M0[m] = sums[3 + m] * (h->dz * h->dv); d->dM0[m] = d->M0[m] - h->M0_init[m]; }
+  d->trace_dev_max = maxs[1];
+  d->ex_abs_max = maxs[2];
+  return COSENU_OK;
+}
+
+extern "C" int64_t cosenu_launch_count(const cosenu_t* h) { return h ? h->launches : 0; }
+
+extern "C" int cosenu_stage_times(cosenu_t* h, double* ms_sum, int64_t* launches_per_stage) {
+  if (!h || !ms_sum || !launches_per_stage) return COSENU_EINVAL;
+  int rc = drain_events(h);
+  if (rc) return rc;
+  for (int k = 0; k < 4; ++k) { ms_sum[k] = h->stage_ms[k]; h->stage_ms[k] = 0; }
+  *launches_per_stage = h->stage_n; h->stage_n = 0;
+  return COSENU_OK;
+}
+
+extern "C" void cosenu_destroy(cosenu_t* h) {
+  if (!h) return;
+  cudaSetDevice(h->device);
+  if (h->maps_ready) cudaStreamSynchronize(h->stream);
+  for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
+  if (h->ws_owned && h->ws) cudaFree(h->ws);
+  delete h;
+}
+
+extern "C" const char* cosenu_last_error(const cosenu_t* h) { return h ? h->err.c_str() : g_create_err.c_str(); }

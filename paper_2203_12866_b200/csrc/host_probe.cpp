@@ -1,0 +1,12 @@
+// host_probe.cpp -- host-side build of the product's stencil arithmetic (weno7_math.h) so that the CPU
+// tests can check the formulas the kernels use against the oracle without a GPU.  Not used by the product.
+#include "weno7_math.h"
+
+extern "C" double cosenu_probe_weno7_face(const double* w7, double v, double eps) {
+  // value of f = v u at the interface, as the kernels form it
+  return v * cosenu_math::weno7_face(w7, v * v, eps);
+}
+
+extern "C" double cosenu_probe_fd4_ko3(const double* u5, double v, double dz, double eps_ko) {
+  return cosenu_math::fd4_ko3(u5[0], u5[1], u5[2], u5[3], u5[4], -v / (12.0 * dz), -eps_ko / (16.0 * dz));
+}

@@ -1,0 +1,105 @@
+// weno7_math.h -- per-interface arithmetic of the product's WENO7 and FD4+KO3 stencils.
+//
+// Compiles as CUDA device code (stage_kernels.cuh) and as plain host C++ (host_probe.cpp, used only by
+// the CPU tests to check these formulas without a GPU).  Shares nothing with oracle/.
+//
+// WENO7 (App. A / Algorithm 1; Eqs. (12)-(14) PAPER.md:134-145).
+// The paper prints the smoothness indicators SI_r as 10-term polynomials in the four cell values of
+// sub-stencil S_r (Eq. A.3).  They vanish on constants, so they are quadratic forms in the three
+// undivided first differences x, y, z of S_r.  Writing the cubic p_r(xi) = a0 + a1 xi + a2 xi^2 + a3 xi^3
+// that has the four cell averages of S_r (xi in cell widths, centred on cell i), the printed SI_r are
+// exactly 240 * sum_{l=1..3} int_{-1/2}^{1/2} (d^l p_r / d xi^l)^2 d xi, which diagonalises to
+//      SI_r = 240 A_r^2 + 260 s_r^2 + (781/3) t_r^2,
+//      A_r = a1 + a3/4,   s_r = 2 a2,   t_r = 6 a3 (the third difference of S_r),
+// and the 4th-order candidate of Eq. (A.2) is   fhat_r = u_i + A_r/2 + s_r/12.
+// (Derived for this file from the printed coefficients; the derivation is restated in DESIGN.md.)
+// With p = y - x, q = z - y (second differences), t = q - p:
+//      r=0 (S_0 = i..i+3):   A = x - (5/6)p + (1/3)q,   s = p - t
+//      r=1 (S_1 = i-1..i+2): A = x + (2/3)p - (1/6)q,   s = p
+//      r=2 (S_2 = i-2..i+1): A = x + (7/6)p + (1/3)q,   s = q
+//      r=3 (S_3 = i-3..i):   A = x + (2/3)p + (11/6)q,  s = q + t
+// The difference form needs ~80 fp64 instructions per interface instead of ~140 and has no
+// catastrophic cancellation for nearly constant data.
+//
+// Linear weights (PAPER.md:372 prints them in the reverse order of its own r labels; only
+// d_0..d_3 = 4/35, 18/35, 12/35, 1/35 reproduces Eq. (A.1), reading A6).
+//
+// The reconstruction acts on f = v u with v constant along z (reading A8), so
+// SI_r[f] = v^2 SI_r[u] and  fhat[f] = v fhat[u]:  the routine works on u and takes v^2.
+// The nonlinear weights  w_r = d_r / (SI_r + eps)^2  (Eq. 14) are combined with ONE division:
+//      F = sum_r w_r fhat_r / sum_r w_r = u_i + (1/2) [sum_r W_r (A_r + s_r/6)] / [sum_r W_r],
+//      W_r = d_r prod_{m != r} (SI_m + eps)^2.
+#ifndef COSENU_WENO7_MATH_H
+#define COSENU_WENO7_MATH_H
+
+#ifdef __CUDACC__
+#define COSENU_HD __host__ __device__ __forceinline__
+#else
+#include <cmath>
+#define COSENU_HD inline
+using std::fma;
+#endif
+
+namespace cosenu_math {
+
+// reciprocal to ~1 ulp: hardware seed + 2 Newton steps on the device, plain division on the host
+COSENU_HD double fast_rcp(double d) {
+#ifdef __CUDA_ARCH__
+  double x;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(d));
+  double e = fma(-d, x, 1.0);
+  x = fma(x, e, x);
+  e = fma(-d, x, 1.0);
+  x = fma(x, e, x);
+  e = fma(-d, x, 1.0);
+  x = fma(x, e, x);
+  return x;
+#else
+  return 1.0 / d;
+#endif
+}
+
+// WENO7 value of u at the interface between w[3] and w[4], biased towards w[0] (the upwind side):
+// w[0..6] = u_{i-3} .. u_{i+3} for v >= 0; the mirrored cells u_{i+4} .. u_{i-2} for v < 0.
+// v2 = v^2, eps = epsilon of Eq. (14).
+COSENU_HD double weno7_face(const double w[7], double v2, double eps) {
+  const double D0 = w[1] - w[0], D1 = w[2] - w[1], D2 = w[3] - w[2], D3 = w[4] - w[3], D4 = w[5] - w[4],
+               D5 = w[6] - w[5];
+  const double E0 = D1 - D0, E1 = D2 - D1, E2 = D3 - D2, E3 = D4 - D3, E4 = D5 - D4;
+  const double T0 = E1 - E0, T1 = E2 - E1, T2 = E3 - E2, T3 = E4 - E3;
+  // A_r, s_r per sub-stencil (x, p, q, t) = (D[3-r], E[3-r], E[4-r], T[3-r])
+  const double A0 = fma(1.0 / 3.0, E4, fma(-5.0 / 6.0, E3, D3));
+  const double A1 = fma(-1.0 / 6.0, E3, fma(2.0 / 3.0, E2, D2));
+  const double A2 = fma(1.0 / 3.0, E2, fma(7.0 / 6.0, E1, D1));
+  const double A3 = fma(11.0 / 6.0, E1, fma(2.0 / 3.0, E0, D0));
+  const double s0 = E3 - T3, s1 = E2, s2 = E2, s3 = E1 + T0;
+  const double ca = 240.0 * v2, cs = 260.0 * v2, ct = (781.0 / 3.0) * v2;
+  // q_r = v^2 SI_r[u] + eps
+  const double q0 = fma(ca, A0 * A0, fma(cs, s0 * s0, fma(ct, T3 * T3, eps)));
+  const double q1 = fma(ca, A1 * A1, fma(cs, s1 * s1, fma(ct, T2 * T2, eps)));
+  const double q2 = fma(ca, A2 * A2, fma(cs, s2 * s2, fma(ct, T1 * T1, eps)));
+  const double q3 = fma(ca, A3 * A3, fma(cs, s3 * s3, fma(ct, T0 * T0, eps)));
+  const double Q0 = q0 * q0, Q1 = q1 * q1, Q2 = q2 * q2, Q3 = q3 * q3;
+  const double Q01 = Q0 * Q1, Q23 = Q2 * Q3;
+  const double W0 = (4.0 / 35.0) * (Q1 * Q23), W1 = (18.0 / 35.0) * (Q0 * Q23);
+  const double W2 = (12.0 / 35.0) * (Q01 * Q3), W3 = (1.0 / 35.0) * (Q01 * Q2);
+  const double den = (W0 + W1) + (W2 + W3);
+  const double c0 = fma(1.0 / 6.0, s0, A0), c1 = fma(1.0 / 6.0, s1, A1), c2 = fma(1.0 / 6.0, s2, A2),
+               c3 = fma(1.0 / 6.0, s3, A3);
+  const double num = fma(W0, c0, fma(W1, c1, fma(W2, c2, W3 * c3)));
+  return fma(num, 0.5 * fast_rcp(den), w[3]);
+}
+
+// FD4 + KO3 in difference form (Eq. (5)): returns
+//   cadv * (u_{i-2} - 8u_{i-1} + 8u_{i+1} - u_{i+2}) + cko * (u_{i-2} - 4u_{i-1} + 6u_i - 4u_{i+1} + u_{i+2})
+// with cadv = -v/(12 dz), cko = -eps_ko/(16 dz) (dissipative sign, reading A4).
+// Written on first differences so that z-uniform data gives exactly 0.
+COSENU_HD double fd4_ko3(double um2, double um1, double u0, double up1, double up2, double cadv, double cko) {
+  const double a = um1 - um2, b = u0 - um1, c = up1 - u0, d = up2 - up1;
+  const double central = fma(-7.0, b + c, a + d);        // = -(u_{i-2} - 8u_{i-1} + 8u_{i+1} - u_{i+2})
+  const double fourth = fma(-3.0, c - b, d - a);         // = u_{i+2} - 4u_{i+1} + 6u_i - 4u_{i-1} + u_{i-2}
+  return fma(-cadv, central, cko * fourth);
+}
+
+}  // namespace cosenu_math
+#endif

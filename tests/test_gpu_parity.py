@@ -1,0 +1,220 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs.  Tolerances (BASELINE.json north_star): per-element max abs error <= 1e-12 after 20 steps;
+domain-averaged survival probability within 1e-6 over a run."""
+import numpy as np
+import pytest
+
+from paper_2203_12866_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+FD, FV = 0, 1
+TOL20 = 1e-12
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2203_12866_b200 import binding
+    binding.load()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def R():
+    from oracle import cosenu_ref
+    return cosenu_ref
+
+
+def run_pair(B, R, args, st, nsteps, **opts):
+    g = B.Cosenu(*args, **opts)
+    g.set_state(st)
+    g.step(nsteps)
+    got = g.get_state()
+    gm = g.get_moments()
+    gd = g.diagnostics()
+    g.close()
+    ropts = {k: v for k, v in opts.items() if k in ("eps_ko", "weno_eps", "advect")}
+    r = R.RefSim(*args, **ropts)
+    r.set_state(st)
+    r.step(nsteps)
+    ref = r.get_state()
+    rm = r.moments(ref)
+    rd = r.diagnostics()
+    r.close()
+    return got, ref, gm, rm, gd, rd
+
+
+# ---- sizes: several z-tiles (TZ = 32) and v-chunks (VC = 32 / 16), ragged tails in both directions
+SHAPES = [(64, 16), (1024, 16), (100, 8), (77, 3), (96, 40), (250, 100), (129, 130), (16, 2)]
+
+
+@pytest.mark.parametrize("scheme", [FD, FV])
+@pytest.mark.parametrize("nz,nv", SHAPES)
+def test_one_step_random_state(B, R, scheme, nz, nv):
+    """One RK4 step from an O(1) random (rough) state: every term of the RHS is exercised at full size."""
+    st = inputs.random_state(nz, nv, seed=100 + nz + nv)
+    args = (nz, nv, 0.7 * nz, 0.05, 0.8, 0.3, 1.3, scheme)
+    got, ref, gm, rm, _, _ = run_pair(B, R, args, st, 1)
+    assert np.max(np.abs(got - ref)) <= 2e-14 * max(1.0, np.max(np.abs(ref)))
+    assert np.max(np.abs(gm - rm)) <= 1e-14 * max(1.0, np.max(np.abs(rm)))
+
+
+@pytest.mark.parametrize("scheme", [FD, FV])
+@pytest.mark.parametrize("lean", [False, True])
+def test_20_steps_cfg0_shape(B, R, scheme, lean):
+    """BASELINE config 0 (fast conversion, 1024 x 16, dt = 0.4 dz), 20 steps, both schemes."""
+    c = inputs.CONFIGS["cfg0"]
+    st = inputs.config_state("cfg0")
+    args = (c["nz"], c["nv"], c["L"], c["dt"], c["omega"], c["theta"], c["mu"], scheme)
+    got, ref, gm, rm, gd, rd = run_pair(B, R, args, st, 20, lean_acc=lean)
+    assert np.max(np.abs(got - ref)) <= TOL20
+    assert np.max(np.abs(gm - rm)) <= TOL20
+    assert abs(gd["psurv_nu"] - rd["psurv_nu"]) <= 1e-12
+    assert abs(gd["psurv_nubar"] - rd["psurv_nubar"]) <= 1e-12
+
+
+@pytest.mark.parametrize("scheme", [FD, FV])
+def test_20_steps_large_perturbation(B, R, scheme):
+    """Nonlinear regime from the start (1e-1 seed, smooth + rough content), slow + fast terms on."""
+    nz, nv = 300, 72
+    st = inputs.fast_conversion_state(nz, nv, seed=5, pert_amp=0.1)
+    st += 0.05 * inputs.smooth_random_state(nz, nv, seed=6)
+    args = (nz, nv, float(nz), 0.4, 1e-2, 0.01, 1.0, scheme)
+    got, ref, gm, rm, gd, rd = run_pair(B, R, args, st, 20)
+    assert np.max(np.abs(got - ref)) <= TOL20
+    for k in ("psurv_nu", "psurv_nubar", "dP_max", "dP_avg", "trace_dev_max", "ex_abs_max"):
+        assert abs(gd[k] - rd[k]) <= 1e-11, k
+    assert np.max(np.abs(np.array(gd["M0"]) - np.array(rd["M0"]))) <= 1e-11
+    assert np.max(np.abs(np.array(gd["dM0"]) - np.array(rd["dM0"]))) <= 1e-11
+
+
+def test_vacuum_cfg1_shape_short(B, R):
+    """BASELINE config 1 shape (vacuum only, 4096 x 64) for 20 steps against the oracle."""
+    c = inputs.CONFIGS["cfg1"]
+    st = inputs.config_state("cfg1")
+    args = (c["nz"], c["nv"], c["L"], c["dt"], c["omega"], c["theta"], c["mu"], c["scheme"])
+    got, ref, *_ = run_pair(B, R, args, st, 20)
+    assert np.max(np.abs(got - ref)) <= TOL20
+
+
+def test_weno_cfg2_rows_sampled(B, R):
+    """BASELINE config 2 shape in v (nv = 128) on a z-reduced grid, 20 steps (the oracle's cost scales with nz)."""
+    c = inputs.CONFIGS["cfg2"]
+    nz = 2048
+    st = inputs.config_state("cfg2", nz=nz)
+    args = (nz, c["nv"], float(nz), c["dt"], c["omega"], c["theta"], c["mu"], c["scheme"])
+    got, ref, *_ = run_pair(B, R, args, st, 20)
+    assert np.max(np.abs(got - ref)) <= TOL20
+
+
+@pytest.mark.parametrize("scheme", [FD, FV])
+def test_commutator_only(B, R, scheme):
+    nz, nv = 64, 24
+    st = inputs.random_state(nz, nv, seed=9)
+    args = (nz, nv, 64.0, 0.01, 0.7, 0.4, 2.0, scheme)
+    got, ref, *_ = run_pair(B, R, args, st, 10, advect=False)
+    assert np.max(np.abs(got - ref)) <= 1e-13
+
+
+def test_weno_linear_limit_option(B, R):
+    nz, nv = 128, 32
+    st = inputs.smooth_random_state(nz, nv, seed=3)
+    args = (nz, nv, 128.0, 0.3, 0.0, 0.0, 0.0, FV)
+    got, ref, *_ = run_pair(B, R, args, st, 10, weno_eps=1e30)
+    assert np.max(np.abs(got - ref)) <= 1e-13
+
+
+def test_eps_ko_option(B, R):
+    nz, nv = 128, 16
+    st = inputs.random_state(nz, nv, seed=4)
+    args = (nz, nv, 128.0, 0.3, 0.0, 0.0, 0.5, FD)
+    got, ref, *_ = run_pair(B, R, args, st, 5, eps_ko=0.37)
+    assert np.max(np.abs(got - ref)) <= 1e-13
+
+
+def test_init_matches_oracle_init(B, R):
+    """cosenu_init (library-side generator) gives bit-identical states to the oracle's and the input module's."""
+    for kind in (0, 1, 2):
+        g = B.Cosenu(512, 20, 512.0, 0.4, 0.0, 0.0, 1.0, FV)
+        g.init(12866, pert_amp=1e-2 if kind == 2 else 1e-6, pert_kind=kind)
+        a = g.get_state()
+        g.close()
+        r = R.RefSim(512, 20, 512.0, 0.4, 0.0, 0.0, 1.0, FV)
+        r.init(12866, pert_amp=1e-2 if kind == 2 else 1e-6, pert_kind=kind)
+        b = r.get_state()
+        r.close()
+        assert np.array_equal(a, b), kind
+    # the numpy recipe differs from the C generators only by libm-vs-numpy rounding of cos/sin/exp
+    np.testing.assert_allclose(_init_state(B, 512, 20, 12866), inputs.fast_conversion_state(512, 20, 12866),
+                               rtol=1e-14, atol=1e-21)
+
+
+def _init_state(B, nz, nv, seed):
+    g = B.Cosenu(nz, nv, float(nz), 0.4, 0.0, 0.0, 1.0, FD)
+    g.init(seed)
+    a = g.get_state()
+    g.close()
+    return a
+
+
+def test_state_roundtrip_and_errors(B):
+    nz, nv = 48, 6   # nv not a multiple of 4: padded pitch on the device
+    st = inputs.random_state(nz, nv, seed=1)
+    g = B.Cosenu(nz, nv, 1.0, 0.01, 0.0, 0.0, 0.0, FD)
+    with pytest.raises(B.CosenuError) as e:
+        g.step(1)
+    assert e.value.code == B.ESTATE
+    g.set_state(st, t=2.5)
+    assert np.array_equal(g.get_state(), st)
+    d = g.diagnostics()
+    assert d["t"] == 2.5 and d["step"] == 0
+    g.step(0)
+    assert np.array_equal(g.get_state(), st)
+    with pytest.raises(B.CosenuError):
+        g.set_option(99, 1.0)
+    with pytest.raises(B.CosenuError):
+        g.step(-1)
+    g.close()
+    with pytest.raises(B.CosenuError):
+        B.Cosenu(8, 4, 1.0, 0.1, 0, 0, 0, FD)      # nz < 16
+    with pytest.raises(B.CosenuError):
+        B.Cosenu(64, 4, 1.0, 0.1, 0, 0, 0, 7)      # bad scheme
+
+
+def test_library_owned_workspace(B, R):
+    """Without cosenu_attach the library allocates its own workspace and uses the default stream."""
+    nz, nv = 96, 16
+    st = inputs.random_state(nz, nv, seed=2)
+    args = (nz, nv, 96.0, 0.1, 0.1, 0.2, 1.0, FD)
+    got, ref, *_ = run_pair(B, R, args, st, 3, use_torch_workspace=False)
+    assert np.max(np.abs(got - ref)) <= 1e-13
+
+
+def test_bitwise_reproducible(B):
+    nz, nv = 320, 96
+    st = inputs.fast_conversion_state(nz, nv, seed=8, pert_amp=1e-2)
+    outs = []
+    for _ in range(2):
+        g = B.Cosenu(nz, nv, float(nz), 0.4, 0.0, 0.0, 1.0, FV)
+        g.set_state(st)
+        g.step(10)
+        outs.append(g.get_state())
+        g.close()
+    assert np.array_equal(outs[0], outs[1])
+
+
+def test_invariants_long_run_gpu(B):
+    """Properties that hold at any size (used again at the bench sizes): M0 conserved to rounding for omega = 0
+    (PAPER.md:247-249), trace constant, |P| drift small."""
+    nz, nv = 2048, 64
+    for scheme in (FD, FV):
+        g = B.Cosenu(nz, nv, float(nz), 0.4, 0.0, 0.0, 1.0, scheme)
+        g.init(77, pert_amp=1e-3)
+        g.step(400)
+        d = g.diagnostics()
+        g.close()
+        assert max(abs(x) for x in d["dM0"]) <= 1e-11 * nz
+        assert np.isfinite(d["psurv_nu"]) and 0.0 < d["psurv_nu"] <= 1.0 + 1e-9
