@@ -1,0 +1,298 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the COSEnu RK4 hot path on B200 (one JSON line on stdout).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4] [--impl ours|reference]
+
+A "step" is one classical RK4 step (4 fused stage launches) of the whole (z,v) grid.  metric =
+(z,v) cell-updates per second per RK4 step, fp64.  Default workload: BASELINE.json configs[4]
+(WENO7, 262144 x 512), the largest single-GPU configuration, on which the north-star target is quoted;
+`--workload cfg3` is the bandwidth-scale FD4+KO3 run.  Inputs are seeded and synthetic
+(paper_2203_12866_b200/inputs.py); the state (>= 2 GB per copy) is far larger than L2, so no L2 flush
+is needed between steps.
+
+N > 1 (torchrun): every rank owns an independent replica of the workload on its own GPU (weak scaling,
+no data-path collective: the z-slab halo exchange is a NEXT item); barrier +
+max-over-ranks timing; value = total cells of all ranks / that time.
+
+--impl reference: the CPU oracle (oracle/, as it stands) timed on the host cores on a bounded sample of
+the same workload (rank 0 only).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "(z,v) cell-updates/sec per RK4 step (fp64)"
+UNIT = "cell-updates/s"
+# algorithmic HBM bytes per cell per stage launch:
+# read stage input + u0 + acc, write stage output + acc, 64 B each
+BYTES_PER_CELL_STAGE = {"first": 192, "mid": 320, "last": 192}
+BYTES_PER_CELL_STEP = 1024
+# dram__bytes_read.sum + dram__bytes_write.sum per MID-stage launch from the committed ncu capture
+# (profiles/), per workload; None until captured
+NCU_TRAFFIC_BYTES = {}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.p = index, None
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "50"],
+                                      stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        try:
+            out, _ = self.p.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+            out, _ = self.p.communicate()
+        sm, mx, reasons, pw = [], [], set(), []
+        for line in out.splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def workload(name):
+    from paper_2203_12866_b200 import inputs
+    c = dict(inputs.CONFIGS[name])
+    c["name"] = name
+    return c
+
+
+def oracle_sample(c, target_s=15.0, max_nz=4096):
+    """Time the oracle, as it stands, on a z-reduced sample of workload c (same nv, scheme, physics)."""
+    import numpy as np
+    from oracle import cosenu_ref as R
+    from paper_2203_12866_b200 import inputs
+    nz = min(c["nz"], max_nz)
+    cores = os.cpu_count() or 1
+    st = inputs.config_state(c["name"], nz=nz)
+    r = R.RefSim(nz, c["nv"], float(nz) * (c["L"] / c["nz"]), c["dt"], c["omega"], c["theta"], c["mu"], c["scheme"])
+    r.set_state(st)
+    t0 = time.perf_counter(); r.step(1); t1 = time.perf_counter() - t0      # also the warm-up
+    n = int(max(1, min(200, target_s / max(t1, 1e-3))))
+    t0 = time.perf_counter(); r.step(n); dt = time.perf_counter() - t0
+    r.close()
+    return {"value": nz * c["nv"] * n / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": "%s with nz reduced to %d (nv=%d), %d RK4 steps, OpenMP over z on %d threads, %.1f s"
+                      % (c["name"], nz, c["nv"], n, cores, dt)}, nz, n, dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    c = workload(args.workload)
+    per_step_target = 4.0
+    vals = []
+    import numpy as np
+    from oracle import cosenu_ref as R
+    from paper_2203_12866_b200 import inputs
+    nz = min(c["nz"], 2048)
+    st = inputs.config_state(c["name"], nz=nz)
+    r = R.RefSim(nz, c["nv"], float(nz) * (c["L"] / c["nz"]), c["dt"], c["omega"], c["theta"], c["mu"], c["scheme"])
+    r.set_state(st)
+    for _ in range(args.warmup):
+        r.step(1)
+    t0 = time.perf_counter()
+    r.step(args.steps)
+    dt = time.perf_counter() - t0
+    r.close()
+    cores = os.cpu_count() or 1
+    val = nz * c["nv"] * args.steps / dt
+    sample = "%s with nz reduced to %d (nv=%d): each step = one RK4 step of that sample; OpenMP over z, %d threads" % (
+        c["name"], nz, c["nv"], cores)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": c["name"], "scheme": "FV_WENO7" if c["scheme"] else "FD4_KO3", "nz": c["nz"],
+                   "nv": c["nv"], "sample_nz": nz},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2203_12866_b200 import binding as B
+    from paper_2203_12866_b200 import inputs
+
+    c = workload(args.workload)
+    nz, nv = c["nz"], c["nv"]
+    cells = nz * nv
+    # ---- synthetic seeded input, built on the host in pinned memory (the e2e leg copies from it)
+    host = torch.empty((8, nz, nv), dtype=torch.float64, pin_memory=True)
+    hnp = host.numpy()
+    hnp[...] = inputs.fast_conversion_state(nz, nv, c["seed"] + rank) if c["kind"] == "fast" else \
+        inputs.vacuum_check_state(nz, nv, c["seed"] + rank)
+    sim = B.Cosenu(nz, nv, c["L"], c["dt"], c["omega"], c["theta"], c["mu"], c["scheme"], lean_acc=bool(args.lean_acc))
+    sim.set_state(host)
+    d0 = sim.diagnostics()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident throughput: W warm-up steps, then exactly K timed steps
+    sim.step(args.warmup)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.15)
+    sim.set_option(B.OPT_STAGE_TIMING, 1)       # CUDA events around every stage launch, on the launching stream
+    l0 = sim.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    sim.step(args.steps)
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = sim.launch_count() - l0
+    stage_ms, nst = sim.stage_times()
+    sim.set_option(B.OPT_STAGE_TIMING, 0)
+    clocks = sampler.stop() if rank == 0 else None
+    if world > 1:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * cells * args.steps / (ms * 1e-3)
+
+    # ---- invariants at the bench size (properties that hold at any size)
+    d1 = sim.diagnostics()
+    checks = {"steps_total": d1["step"], "dM0_max": max(abs(x) for x in d1["dM0"]),
+              "psurv_nu": d1["psurv_nu"], "trace_dev_max": d1["trace_dev_max"], "dP_max": d1["dP_max"]}
+
+    # ---- end to end through the public API with HOST buffers: H2D of the state, one RK4 step, D2H of the result
+    ne2e = max(1, args.e2e_steps)
+    sim.set_state(host); sim.step(1); sim.get_state(host)     # warm-up of the e2e path
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(ne2e):
+        sim.set_state(host)
+        sim.step(1)
+        sim.get_state(host)       # synchronises
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    state_bytes = 8 * cells * 8
+    e2e = {"value": world * cells * ne2e / e2e_s, "unit": UNIT, "h2d_bytes_per_step": state_bytes,
+           "d2h_bytes_per_step": state_bytes, "steps": ne2e,
+           "what": "cosenu_set_state(pinned host) + cosenu_step(1) + cosenu_get_state(pinned host) per step"}
+    sim.close()
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    # ---- roofline of the dominant kernel: the MID stage launch (stages 2 and 3: 320 B/cell algorithmic)
+    peak, peak_src = measured_peaks()
+    mid_ms = (stage_ms[1] + stage_ms[2]) / (2.0 * max(nst, 1))
+    kinds = ["first", "mid", "mid", "last"]
+    per_stage = [{"stage": k + 1, "avg_ms": stage_ms[k] / max(nst, 1),
+                  "GBps": BYTES_PER_CELL_STAGE[kinds[k]] * cells / (stage_ms[k] / max(nst, 1) * 1e-3) / 1e9}
+                 for k in range(4)] if nst else []
+    mid_bytes = (256 if args.lean_acc else 320)
+    achieved = mid_bytes * cells / (mid_ms * 1e-3) / 1e9 if nst else None
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak if achieved else None,
+                "traffic": NCU_TRAFFIC_BYTES.get(c["name"]), "peak_source": peak_src,
+                "kernel": "stage_kernel<%s, MID> (RK stages 2 and 3)" % ("WENO7" if c["scheme"] else "FD4_KO3"),
+                "algorithmic_bytes_per_launch": mid_bytes * cells, "avg_launch_ms": mid_ms,
+                "stage_kernel_share_of_step": sum(stage_ms) / max(nst, 1) / (ms / args.steps) if nst else None,
+                "per_stage": per_stage,
+                "step_model_GBps": (896 if args.lean_acc else BYTES_PER_CELL_STEP) * value / world / 1e9,
+                "step_model_frac": (896 if args.lean_acc else BYTES_PER_CELL_STEP) * value / world / 1e9 / peak}
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        cpu, _, _, _ = oracle_sample(c)
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f64", "data": "synthetic",
+           "config": {"workload": c["name"], "scheme": "FV_WENO7" if c["scheme"] else "FD4_KO3", "nz": nz, "nv": nv,
+                      "dt": c["dt"], "omega": c["omega"], "theta": c["theta"], "mu": c["mu"],
+                      "state_bytes_per_copy": state_bytes, "l2": "inputs larger than L2 (no flush needed)",
+                      "parallelism": "replicas x%d" % world, "lean_acc": bool(args.lean_acc)},
+           "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+           "checks": checks}
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="cfg4", choices=["cfg0", "cfg1", "cfg2", "cfg3", "cfg4"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--lean-acc", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
