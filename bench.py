@@ -175,7 +175,8 @@ def run_ours(args):
     hnp = host.numpy()
     hnp[...] = inputs.fast_conversion_state(nz, nv, c["seed"] + rank) if c["kind"] == "fast" else \
         inputs.vacuum_check_state(nz, nv, c["seed"] + rank)
-    sim = B.Cosenu(nz, nv, c["L"], c["dt"], c["omega"], c["theta"], c["mu"], c["scheme"], lean_acc=bool(args.lean_acc))
+    sim = B.Cosenu(nz, nv, c["L"], c["dt"], c["omega"], c["theta"], c["mu"], c["scheme"], lean_acc=bool(args.lean_acc),
+                   variant=args.variant)
     sim.set_state(host)
     d0 = sim.diagnostics()
 
@@ -267,7 +268,7 @@ def run_ours(args):
            "config": {"workload": c["name"], "scheme": "FV_WENO7" if c["scheme"] else "FD4_KO3", "nz": nz, "nv": nv,
                       "dt": c["dt"], "omega": c["omega"], "theta": c["theta"], "mu": c["mu"],
                       "state_bytes_per_copy": state_bytes, "l2": "inputs larger than L2 (no flush needed)",
-                      "parallelism": "replicas x%d" % world, "lean_acc": bool(args.lean_acc)},
+                      "parallelism": "replicas x%d" % world, "lean_acc": bool(args.lean_acc), "variant": args.variant},
            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
            "checks": checks}
     print(json.dumps(out))
@@ -284,6 +285,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--lean-acc", type=int, default=0)
+    ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":

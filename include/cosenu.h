@@ -55,8 +55,10 @@ enum {
   COSENU_OPT_LEAN_ACC = 3, /* 1: stage 1 does not store the RK accumulator, stage 2 rebuilds k1 from
                               (y2 - u0) 2/dt  (896 instead of 1024 B of traffic per cell-step, costs
                               <= 1 ulp of the state per step); default 0 */
-  COSENU_OPT_STAGE_TIMING = 4 /* 1: bracket every stage launch with CUDA events on the handle's stream
+  COSENU_OPT_STAGE_TIMING = 4, /* 1: bracket every stage launch with CUDA events on the handle's stream
                               (read with cosenu_stage_times); default 0 */
+  COSENU_OPT_VARIANT = 5   /* kernel shape: 0 = 16 compute warps x 1 row (default), 1 = 8 compute warps x 2 rows;
+                              same arithmetic per cell, different summation grouping of the moments only */
 };
 
 /* Diagnostics.  References are taken when a state is set. */

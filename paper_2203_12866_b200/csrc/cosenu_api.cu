@@ -23,9 +23,9 @@ typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_
                                     const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                     CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-// tile shapes: TZ rows per CTA, NSEG z-segments, VC beams per chunk
-constexpr int FD_TZ = 32, FD_NSEG = 8;
-constexpr int WN_TZ = 32, WN_NSEG = 8;
+// tile shapes: TZ rows per tile, NSEG compute warps (S = TZ/NSEG rows each),
+// NY / NUA ring depths of the stage-input and of the u0/acc shared-memory slots.  `variant` picks a row.
+constexpr int TZ_ALL = 16;
 constexpr int DIAG_BLOCKS = 592, DIAG_THREADS = 256, REF_BLOCKS = 148;
 
 std::string g_create_err;
@@ -41,7 +41,8 @@ struct cosenu {
   int advect = 1, lean_acc = 0, stage_timing = 0;
   double dz, dv;
   int device = 0;
-  int vc = 32, tz = 32;  // chunk width, rows per CTA
+  int variant = 0;       // kernel shape variant (COSENU_OPT_VARIANT)
+  int num_sms = 148;
 
   // workspace
   void* ws = nullptr; size_t ws_bytes = 0; bool ws_owned = false;
@@ -51,7 +52,8 @@ struct cosenu {
   double *d_pref = nullptr, *d_p0ref = nullptr, *d_refpart = nullptr, *d_diagpart = nullptr;
   int64_t comp_stride = 0; size_t state_elems = 0;
   int mcur = 0;  // M[mcur] holds the moments of U
-  CUtensorMap tm_U, tm_Y1, tm_Y2;
+  CUtensorMap tm_U, tm_Y1, tm_Y2;   // stage-input boxes [8][TZ+2H][32]
+  CUtensorMap tp_U, tp_ACC;         // plain boxes [8][TZ][32] (u0, RK accumulator)
   bool maps_ready = false;
 
   bool have_state = false;
@@ -104,7 +106,7 @@ size_t workspace_layout(const cosenu* h, size_t off[10]) {
 int make_map(cosenu* h, PFN_encodeTiled enc, CUtensorMap* map, double* base, int rows_box) {
   const cuuint64_t gdim[3] = {(cuuint64_t)h->nv, (cuuint64_t)(h->nz + 2 * G), 8};
   const cuuint64_t gstr[2] = {(cuuint64_t)h->nvp * 8, (cuuint64_t)h->comp_stride * 8};
-  const cuuint32_t box[3] = {(cuuint32_t)h->vc, (cuuint32_t)rows_box, 8};
+  const cuuint32_t box[3] = {(cuuint32_t)VC, (cuuint32_t)rows_box, 8};
   const cuuint32_t estr[3] = {1, 1, 1};
   CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, base, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                    CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
@@ -135,49 +137,53 @@ int ensure_workspace(cosenu* h) {
   CK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr));
   if (!fn || qr != cudaDriverEntryPointSuccess) return fail(h, COSENU_ECUDA, "cuTensorMapEncodeTiled not available in this driver");
   PFN_encodeTiled enc = reinterpret_cast<PFN_encodeTiled>(fn);
-  const int rows = h->tz + 2 * (h->scheme == COSENU_FD4_KO3 ? 2 : 4);
+  const int rows = TZ_ALL + 2 * (h->scheme == COSENU_FD4_KO3 ? 2 : 4);
   int rc;
   if ((rc = make_map(h, enc, &h->tm_U, h->U, rows))) return rc;
   if ((rc = make_map(h, enc, &h->tm_Y1, h->Y1, rows))) return rc;
   if ((rc = make_map(h, enc, &h->tm_Y2, h->Y2, rows))) return rc;
+  if ((rc = make_map(h, enc, &h->tp_U, h->U, TZ_ALL))) return rc;
+  if ((rc = make_map(h, enc, &h->tp_ACC, h->ACC, TZ_ALL))) return rc;
   h->maps_ready = true;
   return COSENU_OK;
 }
 
-template <int SCHEME, int KIND, int TZ, int NSEG, int VC>
+template <int SCHEME, int KIND, int TZ, int NSEG, int NY, int NUA>
 int launch_one(cosenu* h, const CUtensorMap& map, const StageParams& p) {
-  auto kern = stage_kernel<SCHEME, KIND, TZ, NSEG, VC>;
-  constexpr size_t smem = StageSmem<SCHEME, TZ, VC>::bytes;
-  static bool configured = false;  // per instantiation; attributes are per-function and per-context
+  auto kern = stage_kernel<SCHEME, KIND, TZ, NSEG, NY, NUA>;
+  constexpr size_t smem = StageSmem<SCHEME, KIND, TZ, NSEG, NY, NUA>::bytes;
+  static_assert(smem <= 232448, "over the 227 KB shared-memory limit of a CTA");
+  static bool configured = false;  // per instantiation
   if (!configured) {
     CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     configured = true;
   }
-  const unsigned grid = (unsigned)((h->nz + TZ - 1) / TZ);
-  kern<<<grid, NSEG * VC, smem, h->stream>>>(map, p);
+  const long long ntiles = (h->nz + TZ - 1) / TZ;
+  const unsigned grid = (unsigned)(ntiles < h->num_sms ? ntiles : h->num_sms);   // persistent: one CTA per SM
+  kern<<<grid, NSEG * 32 + 32, smem, h->stream>>>(map, h->tp_U, h->tp_ACC, p);
   CK(cudaGetLastError());
   h->launches++;
   return COSENU_OK;
 }
 
-template <int SCHEME, int TZ, int NSEG, int VC>
+template <int SCHEME, int TZ, int NSEG, int NY, int NUA>
 int launch_kind(cosenu* h, int kind, const CUtensorMap& map, const StageParams& p) {
   switch (kind) {
-    case FIRST: return launch_one<SCHEME, FIRST, TZ, NSEG, VC>(h, map, p);
-    case FIRST_LEAN: return launch_one<SCHEME, FIRST_LEAN, TZ, NSEG, VC>(h, map, p);
-    case MID: return launch_one<SCHEME, MID, TZ, NSEG, VC>(h, map, p);
-    case MID_REBUILD: return launch_one<SCHEME, MID_REBUILD, TZ, NSEG, VC>(h, map, p);
-    default: return launch_one<SCHEME, LAST, TZ, NSEG, VC>(h, map, p);
+    case FIRST: return launch_one<SCHEME, FIRST, TZ, NSEG, NY, NUA>(h, map, p);
+    case FIRST_LEAN: return launch_one<SCHEME, FIRST_LEAN, TZ, NSEG, NY, NUA>(h, map, p);
+    case MID: return launch_one<SCHEME, MID, TZ, NSEG, NY, NUA>(h, map, p);
+    case MID_REBUILD: return launch_one<SCHEME, MID_REBUILD, TZ, NSEG, NY, NUA>(h, map, p);
+    default: return launch_one<SCHEME, LAST, TZ, NSEG, NY, NUA>(h, map, p);
   }
 }
 
 int launch_stage(cosenu* h, int kind, const CUtensorMap& map, const StageParams& p) {
   if (h->scheme == COSENU_FD4_KO3) {
-    if (h->vc == 16) return launch_kind<0, FD_TZ, 2 * FD_NSEG, 16>(h, kind, map, p);
-    return launch_kind<0, FD_TZ, FD_NSEG, 32>(h, kind, map, p);
+    if (h->variant == 1) return launch_kind<0, TZ_ALL, 8, 2, 2>(h, kind, map, p);
+    return launch_kind<0, TZ_ALL, 16, 2, 2>(h, kind, map, p);
   }
-  if (h->vc == 16) return launch_kind<1, WN_TZ, 2 * WN_NSEG, 16>(h, kind, map, p);
-  return launch_kind<1, WN_TZ, WN_NSEG, 32>(h, kind, map, p);
+  if (h->variant == 1) return launch_kind<1, TZ_ALL, 8, 2, 1>(h, kind, map, p);
+  return launch_kind<1, TZ_ALL, 16, 2, 1>(h, kind, map, p);
 }
 
 StageParams base_params(const cosenu* h) {
@@ -235,12 +241,12 @@ int one_step(cosenu* h) {
   double* Min = h->M[h->mcur];
   double* Mout = h->M[h->mcur ^ 1];
   // stage 1: k1 = RHS(U); Y1 = U + dt/2 k1; ACC = U + dt/6 k1
-  p.u0 = nullptr; p.acc_in = nullptr; p.y_out = h->Y1; p.acc_out = h->ACC; p.mom_in = Min; p.mom_out = Mout;
+  p.y_out = h->Y1; p.acc_out = h->ACC; p.mom_in = Min; p.mom_out = Mout;
   p.cy = 0.5 * dt; p.ca = dt / 6.0;
   if ((rc = launch_stage(h, h->lean_acc ? FIRST_LEAN : FIRST, h->tm_U, p))) return rc;
   if (tm) CK(cudaEventRecord(ev[1], h->stream));
   // stage 2: k2 = RHS(Y1); Y2 = U + dt/2 k2; ACC += dt/3 k2
-  p.u0 = h->U; p.acc_in = h->ACC; p.y_out = h->Y2; p.acc_out = h->ACC; p.mom_in = Mout; p.mom_out = Min;
+  p.y_out = h->Y2; p.acc_out = h->ACC; p.mom_in = Mout; p.mom_out = Min;
   p.cy = 0.5 * dt; p.ca = dt / 3.0;
   if ((rc = launch_stage(h, h->lean_acc ? MID_REBUILD : MID, h->tm_Y1, p))) return rc;
   if (tm) CK(cudaEventRecord(ev[2], h->stream));
@@ -250,7 +256,7 @@ int one_step(cosenu* h) {
   if ((rc = launch_stage(h, MID, h->tm_Y2, p))) return rc;
   if (tm) CK(cudaEventRecord(ev[3], h->stream));
   // stage 4: k4 = RHS(Y1); U = ACC + dt/6 k4
-  p.u0 = nullptr; p.y_out = h->U; p.acc_out = nullptr; p.mom_in = Mout; p.mom_out = Min;
+  p.y_out = h->U; p.acc_out = nullptr; p.mom_in = Mout; p.mom_out = Min;
   p.cy = dt / 6.0; p.ca = 0.0;
   if ((rc = launch_stage(h, LAST, h->tm_Y1, p))) return rc;
   if (tm) CK(cudaEventRecord(ev[4], h->stream));
@@ -349,8 +355,7 @@ extern "C" cosenu_t* cosenu_create(int64_t nz, int32_t nv, double L, double dt, 
   h->nvp = (nv + 3) / 4 * 4;
   h->dz = L / (double)nz; h->dv = 2.0 / (double)nv;
   h->comp_stride = (int64_t)(nz + 2 * G) * h->nvp;
-  h->vc = nv <= 16 ? 16 : 32;
-  h->tz = scheme == COSENU_FD4_KO3 ? FD_TZ : WN_TZ;
+  h->num_sms = prop.multiProcessorCount;
   return h;
 }
 
@@ -379,6 +384,7 @@ extern "C" int cosenu_set_option(cosenu_t* h, int key, double value) {
     case COSENU_OPT_WENO_EPS: if (!(value > 0) || !(value <= 1e30)) break; h->weno_eps = value; return COSENU_OK;
     case COSENU_OPT_ADVECT: h->advect = value != 0; return COSENU_OK;
     case COSENU_OPT_LEAN_ACC: h->lean_acc = value != 0; return COSENU_OK;
+    case COSENU_OPT_VARIANT: if (value != 0 && value != 1) break; h->variant = (int)value; return COSENU_OK;
     case COSENU_OPT_STAGE_TIMING: {
       int rc = drain_events(h);
       if (rc) return rc;

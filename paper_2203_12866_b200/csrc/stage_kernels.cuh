@@ -1,4 +1,4 @@
-// stage_kernels.cuh -- ONE fused kernel per RK stage (sm_100a, fp64).
+// stage_kernels.cuh -- ONE fused, persistent kernel per RK stage (sm_100a, fp64).
 //
 // Per launch and per (z,v) cell:
 //   advection of the 8 real components by FD4+KO3 or FV-WENO7 (App. A),
@@ -7,15 +7,19 @@
 //   classical RK4 combine,
 //   and, in the epilogue, the 6 velocity moments of the state just produced (the S1 of the next stage).
 //
-// Mapping.  Device layout of a state: double [8][nz + 2G][nvp], v fastest (G = 4 periodic ghost rows on
-// each side of z, nvp = nv rounded up to 4).  One CTA owns TZ consecutive z rows and ALL v: it walks the
-// v axis in chunks of VC beams.  The stage-input tile of a chunk ([8][TZ + 2H][VC] doubles, H = stencil
-// halo) is brought into shared memory by ONE 3-D TMA box (cp.async.bulk.tensor) per chunk, double
-// buffered on mbarriers, so the stencil reads come from shared memory and the load of chunk n+1
-// overlaps the arithmetic of chunk n.  A thread = one beam (lane) x one z-segment of S = TZ/NSEG rows.
-// u0 and the RK accumulator have no reuse and are read straight from global memory, coalesced over v.
-// The moments are reduced over the lanes with shuffles and accumulated per row in shared memory in
-// chunk order (fixed order => bit-reproducible; no atomics).
+// Design.  Device layout of a state: double [8][nz + 2G][nvp], v fastest (G = 4
+// periodic ghost rows on each side of z, nvp = nv rounded up to 4).
+//  * Persistent CTAs (one per SM).  Work item = (z-tile of TZ rows, chunk of 32 beams); a CTA walks the
+//    chunks of its tiles (tile = blockIdx.x + k gridDim.x), so a tile's moments never leave the CTA.
+//  * Warp-specialised: one producer warp feeds shared memory with 3-D TMA boxes (cp.async.bulk.tensor):
+//    the stage-input tile with its stencil halo [8][TZ+2H][32] (ring of NY slots) and the operands that
+//    have no reuse, u0 and the RK accumulator [8][TZ][32] (ring of NUA slots); full/empty mbarriers.
+//    The compute warps never wait on a global load.
+//  * Compute warp w owns rows w*S .. w*S+S-1 of the tile, lane = beam.  WENO7: every interface flux is
+//    computed once; neighbouring warps exchange the flux of their common interface through shared memory
+//    (xfull/xfree mbarriers); the tile's left boundary flux is split by component over 8 warps.
+//  * Moments of the output: butterfly reduce-scatter over the lanes (N values cost ~N adds, not 5N),
+//    accumulated over the chunks in registers of the owning lanes in fixed order => bit-reproducible.
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -25,14 +29,12 @@
 
 namespace cosenu_dev {
 
-constexpr int G = 4;        // ghost rows per side in the device layout
-constexpr int NBUF = 2;     // TMA double buffering
+constexpr int G = 4;    // ghost rows per side in the device layout
+constexpr int VC = 32;  // beams per chunk = lanes of a warp
 
 enum StageKind { FIRST = 0, FIRST_LEAN = 1, MID = 2, MID_REBUILD = 3, LAST = 4 };
 
 struct StageParams {
-  const double* u0;       // U (state at the beginning of the step), device layout; MID kinds only
-  const double* acc_in;   // RK accumulator; MID and LAST
   double* y_out;          // next stage input (FIRST/MID) or the new U (LAST)
   double* acc_out;        // RK accumulator (FIRST, MID kinds)
   const double* mom_in;   // [6][nz] moments of the stage input (already times dv)
@@ -43,19 +45,22 @@ struct StageParams {
   double cy, ca;          // y_out = base + cy k ; acc_out = acc_in + ca k
   double mu, A0, Br0;     // A0 = -omega cos 2theta, Br0 = (omega/2) sin 2theta
   double dv;
-  double cadv, cko;       // FD: -1/(12 dz), -eps_ko/(16 dz)   (times the advect switch)
+  double cadv, cko;          // FD: -1/(12 dz), -eps_ko/(16 dz)   (times the advect switch)
   double ninv_dz, weno_eps;  // WENO: -1/dz (times the advect switch), epsilon of Eq. (14)
 };
 
 // ----------------------------------------------------------------------------- PTX helpers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
 }
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   asm volatile(
       "{\n"
       ".reg .pred p;\n"
@@ -64,148 +69,265 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
       "@p bra DONE_%=;\n"
       "bra WAIT_%=;\n"
       "DONE_%=:\n"
-      "}\n" ::"r"(smem_u32(bar)),
+      "}\n" ::"r"(bar),
       "r"(parity)
       : "memory");
 }
 // 3-D tiled TMA load global -> shared, completion on an mbarrier
-__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2) {
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1, int c2) {
   asm volatile(
-      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];" ::"r"(
-          smem_u32(dst)),
-      "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];" ::"r"(dst),
+      "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2)
       : "memory");
 }
+__device__ __forceinline__ double lds(uint32_t addr) {
+  double v;
+  asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ void sts(uint32_t addr, double v) {
+  asm volatile("st.shared.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory");
+}
 
-template <int SCHEME, int TZ, int VC>
+template <int KIND>
+struct KindTraits {
+  static constexpr bool LOAD_U0 = (KIND == MID || KIND == MID_REBUILD);
+  static constexpr bool LOAD_ACC = (KIND == MID || KIND == LAST);
+  static constexpr bool WRITE_ACC = (KIND == FIRST || KIND == MID || KIND == MID_REBUILD);
+  static constexpr int NARR = (LOAD_U0 ? 1 : 0) + (LOAD_ACC ? 1 : 0);
+};
+
+// shared-memory carve-up (byte offsets from a 128-byte aligned base)
+template <int SCHEME, int KIND, int TZ, int NSEG, int NY, int NUA>
 struct StageSmem {
   static constexpr int H = SCHEME == 0 ? 2 : 4;
   static constexpr int ROWS = TZ + 2 * H;
-  static constexpr int TILE = 8 * ROWS * VC;  // doubles per buffer
-  static constexpr size_t bytes = sizeof(double) * ((size_t)NBUF * TILE + 12 * TZ) + 8 * NBUF + 128;
+  static constexpr uint32_t YTILE = 8u * ROWS * VC * 8u;   // bytes per stage-input slot
+  static constexpr uint32_t PTILE = 8u * TZ * VC * 8u;     // bytes per u0 / acc slot
+  static constexpr int NARR = KindTraits<KIND>::NARR;
+  static constexpr uint32_t off_y = 0;
+  static constexpr uint32_t off_ua = off_y + NY * YTILE;               // [NUA][NARR][PTILE]
+  static constexpr uint32_t off_x = off_ua + NUA * NARR * PTILE;       // [NSEG][8][32] exchange (WENO)
+  static constexpr uint32_t off_xb = off_x + (SCHEME == 1 ? NSEG * 8u * VC * 8u : 0u);  // [8][32] boundary (WENO)
+  static constexpr uint32_t off_bar = off_xb + (SCHEME == 1 ? 8u * VC * 8u : 0u);
+  static constexpr uint32_t nbar = 2 * NY + 2 * NUA + 2;
+  static constexpr size_t bytes = off_bar + 8 * nbar + 128;
 };
 
+// ----------------------------------------------------------------------------- butterfly reduce-scatter
+// Sum each of x[0..N-1] over the 32 lanes.  Stage with lane offset o halves the live values: the lanes with
+// bit o keep the upper half and send the lower half (and vice versa), so N values cost about N adds and
+// N shuffles per lane instead of 5N.  On return x[0] of lane L holds the total of the original value
+// `idx` (if `valid`), idx = sum over stages of (lane bit ? half : 0).  Fixed tree => reproducible.
+template <int N>
+__device__ __forceinline__ void butterfly_reduce(double (&x)[N], int lane, int& idx, bool& valid) {
+  int n = N;
+#pragma unroll
+  for (int o = 16; o >= 1; o >>= 1) {
+    const int half = (n + 1) / 2;
+    const bool up = (lane & o) != 0;
+#pragma unroll
+    for (int i = 0; i < half; ++i) {
+      const double a = x[i];
+      const double b = (i + half < n) ? x[i + half] : 0.0;
+      const double send = up ? a : b;
+      const double keep = up ? b : a;
+      x[i] = keep + __shfl_xor_sync(0xffffffffu, send, o);
+    }
+    n = half;
+  }
+  // which original index ended up in x[0] of this lane (replay the stages backwards)
+  int ns[5], hs[5];
+  n = N;
+#pragma unroll
+  for (int k = 0; k < 5; ++k) { ns[k] = n; hs[k] = (n + 1) / 2; n = hs[k]; }
+  int pos = 0;
+  valid = true;
+#pragma unroll
+  for (int k = 4; k >= 0; --k) {
+    if (lane & (16 >> k)) pos += hs[k];
+    valid = valid && (pos < ns[k]);
+  }
+  idx = pos;
+}
+
 // ----------------------------------------------------------------------------- the stage kernel
-template <int SCHEME, int KIND, int TZ, int NSEG, int VC>
-__global__ void __launch_bounds__(NSEG* VC, 1)
-    stage_kernel(const __grid_constant__ CUtensorMap tmap_y, const StageParams p) {
-  using SM = StageSmem<SCHEME, TZ, VC>;
-  constexpr int H = SM::H, ROWS = SM::ROWS, TILE = SM::TILE;
+template <int SCHEME, int KIND, int TZ, int NSEG, int NY, int NUA>
+__global__ void __launch_bounds__(NSEG * 32 + 32, 1)
+    stage_kernel(const __grid_constant__ CUtensorMap tm_y, const __grid_constant__ CUtensorMap tm_u0,
+                 const __grid_constant__ CUtensorMap tm_acc, const StageParams p) {
+  using SM = StageSmem<SCHEME, KIND, TZ, NSEG, NY, NUA>;
+  using KT = KindTraits<KIND>;
+  constexpr int H = SM::H, ROWS = SM::ROWS;
   constexpr int S = TZ / NSEG;
-  constexpr int NT = NSEG * VC;
-  constexpr bool LOAD_U0 = (KIND == MID || KIND == MID_REBUILD);
-  constexpr bool LOAD_ACC = (KIND == MID || KIND == LAST);
-  constexpr bool WRITE_ACC = (KIND == FIRST || KIND == MID || KIND == MID_REBUILD);
-  static_assert(TZ % NSEG == 0 && VC <= 32 && (32 % VC) == 0, "tile shape");
+  constexpr int NW = NSEG;  // compute warps
+  constexpr int NARR = KT::NARR;
+  static_assert(TZ % NSEG == 0 && 6 * S <= 32, "tile shape");
+  static_assert(SCHEME == 0 || NSEG >= 8, "WENO boundary flux is split over 8 warps");
 
   extern __shared__ unsigned char smem_raw[];
-  double* tile = reinterpret_cast<double*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~uintptr_t(127));
-  double* s_min = tile + NBUF * TILE;   // [6][TZ]  mu * moments of the stage input
-  double* s_macc = s_min + 6 * TZ;      // [6][TZ]  running moments of the output
-  uint64_t* full = reinterpret_cast<uint64_t*>(s_macc + 6 * TZ);
+  const uint32_t sbase = (smem_u32(smem_raw) + 127u) & ~127u;
+  const uint32_t s_y = sbase + SM::off_y, s_ua = sbase + SM::off_ua, s_x = sbase + SM::off_x, s_xb = sbase + SM::off_xb;
+  const uint32_t s_bar = sbase + SM::off_bar;
+  // barriers: full_y[NY], empty_y[NY], full_ua[NUA], empty_ua[NUA], xfull, xfree
+  const uint32_t b_full_y = s_bar, b_empty_y = s_bar + 8 * NY, b_full_ua = s_bar + 16 * NY,
+                 b_empty_ua = s_bar + 16 * NY + 8 * NUA, b_xfull = s_bar + 16 * NY + 16 * NUA, b_xfree = b_xfull + 8;
 
-  const int tid = threadIdx.x;
-  const int lane = tid % VC;
-  const int seg = tid / VC;
-  const long long iz0 = (long long)blockIdx.x * TZ;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int nchunks = (p.nv + VC - 1) / VC;
+  const long long ntiles = (p.nz + TZ - 1) / TZ;
+  const long long my_tiles = blockIdx.x < ntiles ? (ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+  const long long nitems = my_tiles * nchunks;
 
-  if (tid == 0) {
-    for (int b = 0; b < NBUF; ++b) mbar_init(&full[b], 1);
+  if (threadIdx.x == 0) {
+    for (int b = 0; b < NY; ++b) { mbar_init(b_full_y + 8 * b, 1); mbar_init(b_empty_y + 8 * b, NW); }
+    for (int b = 0; b < NUA; ++b) { mbar_init(b_full_ua + 8 * b, 1); mbar_init(b_empty_ua + 8 * b, NW); }
+    mbar_init(b_xfull, NW);
+    mbar_init(b_xfree, NW);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  for (int q = tid; q < 6 * TZ; q += NT) {
-    const int m = q / TZ, r = q - m * TZ;
-    const long long iz = iz0 + r;
-    s_min[q] = iz < p.nz ? p.mu * p.mom_in[(long long)m * p.nz + iz] : 0.0;
-    s_macc[q] = 0.0;
-  }
   __syncthreads();
-  if (tid == 0) {
-    for (int b = 0; b < NBUF && b < nchunks; ++b) {
-      mbar_expect_tx(&full[b], TILE * 8);
-      tma_load_3d(tile + b * TILE, &tmap_y, &full[b], b * VC, (int)(iz0 + G - H), 0);
+
+  // =========================================================================== producer warp
+  if (warp == NW) {
+    if (lane == 0) {
+      long long tile = blockIdx.x;
+      int ch = 0;
+      for (long long n = 0; n < nitems; ++n) {
+        const int iz0 = (int)(tile * TZ);
+        const int sy = (int)(n % NY);
+        mbar_wait(b_empty_y + 8 * sy, (uint32_t)(((n / NY) & 1) ^ 1));
+        mbar_expect_tx(b_full_y + 8 * sy, SM::YTILE);
+        tma_load_3d(s_y + sy * SM::YTILE, &tm_y, b_full_y + 8 * sy, ch * VC, iz0 + G - H, 0);
+        if constexpr (NARR > 0) {
+          const int su = (int)(n % NUA);
+          mbar_wait(b_empty_ua + 8 * su, (uint32_t)(((n / NUA) & 1) ^ 1));
+          mbar_expect_tx(b_full_ua + 8 * su, NARR * SM::PTILE);
+          uint32_t dst = s_ua + su * NARR * SM::PTILE;
+          if constexpr (KT::LOAD_U0) { tma_load_3d(dst, &tm_u0, b_full_ua + 8 * su, ch * VC, iz0 + G, 0); dst += SM::PTILE; }
+          if constexpr (KT::LOAD_ACC) tma_load_3d(dst, &tm_acc, b_full_ua + 8 * su, ch * VC, iz0 + G, 0);
+        }
+        if (++ch == nchunks) { ch = 0; tile += gridDim.x; }
+      }
     }
+    return;
   }
 
-  for (int ch = 0; ch < nchunks; ++ch) {
-    const int buf = ch % NBUF;
-    const double* T = tile + buf * TILE;
+  // =========================================================================== compute warps
+  const int row0 = warp * S;
+  double macc = 0.0;      // running moment (one (row, quantity) per valid lane, see butterfly_reduce)
+  double min_cur = 0.0;   // lane l < 6S: mu * moment (l % 6) of row row0 + l / 6 of the stage input
+  long long tile = blockIdx.x;
+  int ch = 0;
+  for (long long n = 0; n < nitems; ++n) {
+    const long long iz0 = tile * TZ;
+    if (ch == 0) {
+      min_cur = 0.0;
+      if (lane < 6 * S) {
+        const long long iz = iz0 + row0 + lane / 6;
+        if (iz < p.nz) min_cur = p.mu * __ldg(p.mom_in + (long long)(lane % 6) * p.nz + iz);
+      }
+    }
+    const int sy = (int)(n % NY);
+    const uint32_t Ty = s_y + sy * SM::YTILE + lane * 8;   // + ((c * ROWS + r) * 32) * 8
     const int j = ch * VC + lane;
     const bool active = j < p.nv;
     // v_j = -1 + (j + 1/2) dv, formed without contraction
     const double v = __dadd_rn(-1.0, __dmul_rn((double)j + 0.5, p.dv));
-    mbar_wait(&full[buf], (ch / NBUF) & 1);
+    mbar_wait(b_full_y + 8 * sy, (uint32_t)((n / NY) & 1));
 
-    const int row0 = seg * S;
-    double Fprev[8];
-    int wdir = 1;
-    double v2 = 0.0, nvz = 0.0, cadv_v = 0.0;
+    // ---- S2 (WENO7): right-interface fluxes of my rows, exchanged with the neighbouring warps
+    double FR[SCHEME == 1 ? S : 1][8];
+    double FL[8];
+    double nvz = 0.0, cadv_v = 0.0;
     if constexpr (SCHEME == 1) {
-      wdir = v >= 0.0 ? 1 : -1;
-      v2 = v * v;
+      const int wdir = v >= 0.0 ? 1 : -1;
+      const int rsh = wdir > 0 ? 0 : 1;       // centre cell of the upwind-biased stencil: i or i+1
+      const int wstep = wdir * VC * 8;        // byte step of one stencil cell towards the downwind side
+      const double v2 = v * v;
       nvz = v * p.ninv_dz;
-      // flux at the interface on the left of the segment's first cell
-      const int rc = row0 - 1 + H + (wdir > 0 ? 0 : 1);
 #pragma unroll
-      for (int c = 0; c < 8; ++c) {
-        const double* b = T + (c * ROWS + rc) * VC + lane;
+      for (int s = 0; s < S; ++s) {
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+          const uint32_t b = Ty + ((c * ROWS + row0 + s + H + rsh) * VC) * 8;
+          double w[7];
+#pragma unroll
+          for (int k = 0; k < 7; ++k) w[k] = lds(b + (k - 3) * wstep);
+          FR[s][c] = cosenu_math::weno7_face(w, v2, p.weno_eps);
+        }
+      }
+      double FB = 0.0;
+      if (warp < 8) {  // left boundary interface of the tile, component `warp`
+        const uint32_t b = Ty + ((warp * ROWS + H - 1 + rsh) * VC) * 8;
         double w[7];
 #pragma unroll
-        for (int k = 0; k < 7; ++k) w[k] = b[wdir * (k - 3) * VC];
-        Fprev[c] = cosenu_math::weno7_face(w, v2, p.weno_eps);
+        for (int k = 0; k < 7; ++k) w[k] = lds(b + (k - 3) * wstep);
+        FB = cosenu_math::weno7_face(w, v2, p.weno_eps);
       }
+      mbar_wait(b_xfree, (uint32_t)((n & 1) ^ 1));   // readers of the previous item are done
+#pragma unroll
+      for (int c = 0; c < 8; ++c) sts(s_x + ((warp * 8 + c) * VC + lane) * 8, FR[S - 1][c]);
+      if (warp < 8) sts(s_xb + (warp * VC + lane) * 8, FB);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(b_xfull);
     } else {
       cadv_v = v * p.cadv;
     }
 
-#pragma unroll 1
+    // broadcast helper: mu * moment q of my row s
+    auto mom = [&](int s, int q) { return __shfl_sync(0xffffffffu, min_cur, s * 6 + q); };
+
+    if constexpr (SCHEME == 1) {
+      mbar_wait(b_xfull, (uint32_t)(n & 1));
+      if (warp == 0) {
+#pragma unroll
+        for (int c = 0; c < 8; ++c) FL[c] = lds(s_xb + (c * VC + lane) * 8);
+      } else {
+#pragma unroll
+        for (int c = 0; c < 8; ++c) FL[c] = lds(s_x + (((warp - 1) * 8 + c) * VC + lane) * 8);
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(b_xfree);
+    }
+
+    uint32_t Tu = 0, Ta = 0;
+    if constexpr (NARR > 0) {
+      const int su = (int)(n % NUA);
+      Tu = s_ua + su * NARR * SM::PTILE + lane * 8;
+      Ta = Tu + (KT::LOAD_U0 ? SM::PTILE : 0u);
+      mbar_wait(b_full_ua + 8 * su, (uint32_t)((n / NUA) & 1));
+    }
+
+    double mred[6 * S];
+#pragma unroll
     for (int s = 0; s < S; ++s) {
       const int row = row0 + s;
       const long long iz = iz0 + row;
-      const bool valid = iz < p.nz;      // ragged last tile: keep the lanes converged for the shuffles
-      const bool act = active && valid;
-      const int tr = row + H;  // row inside the tile
+      const bool act = active && (iz < p.nz);
+      const int tr = row + H;  // row inside the stage-input tile
       double yc[8], k[8];
 #pragma unroll
-      for (int c = 0; c < 8; ++c) yc[c] = T[(c * ROWS + tr) * VC + lane];
-
-      // global operands with no reuse: issue early
-      const long long gidx = (iz + G) * p.nvp + j;
-      double u0v[8], accv[8];
-#pragma unroll
-      for (int c = 0; c < 8; ++c) {
-        if constexpr (LOAD_U0) u0v[c] = act ? __ldg(p.u0 + c * p.comp_stride + gidx) : 0.0;
-        else u0v[c] = yc[c];
-        if constexpr (LOAD_ACC) accv[c] = act ? __ldg(p.acc_in + c * p.comp_stride + gidx) : 0.0;
-      }
+      for (int c = 0; c < 8; ++c) yc[c] = lds(Ty + ((c * ROWS + tr) * VC) * 8);
 
       // ---- S2: advection
       if constexpr (SCHEME == 0) {
 #pragma unroll
         for (int c = 0; c < 8; ++c) {
-          const double* b = T + (c * ROWS + tr) * VC + lane;
-          k[c] = cosenu_math::fd4_ko3(b[-2 * VC], b[-VC], yc[c], b[VC], b[2 * VC], cadv_v, p.cko);
+          const uint32_t b = Ty + ((c * ROWS + tr) * VC) * 8;
+          k[c] = cosenu_math::fd4_ko3(lds(b - 2 * VC * 8), lds(b - VC * 8), yc[c], lds(b + VC * 8), lds(b + 2 * VC * 8),
+                                      cadv_v, p.cko);
         }
       } else {
-        const int rc = tr + (wdir > 0 ? 0 : 1);
 #pragma unroll
-        for (int c = 0; c < 8; ++c) {
-          const double* b = T + (c * ROWS + rc) * VC + lane;
-          double w[7];
-#pragma unroll
-          for (int q = 0; q < 7; ++q) w[q] = b[wdir * (q - 3) * VC];
-          const double F = cosenu_math::weno7_face(w, v2, p.weno_eps);
-          k[c] = (F - Fprev[c]) * nvz;
-          Fprev[c] = F;
-        }
+        for (int c = 0; c < 8; ++c) k[c] = (FR[s][c] - (s == 0 ? FL[c] : FR[s > 0 ? s - 1 : 0][c])) * nvz;
       }
 
-      // ---- S3: Hamiltonian from the moments (mu folded into s_min), commutator
+      // ---- S3: Hamiltonian from the moments (mu folded in), commutator
       {
-        const double Sd = fma(-v, s_min[1 * TZ + row], s_min[0 * TZ + row]);
-        const double Sr = fma(-v, s_min[3 * TZ + row], s_min[2 * TZ + row]);
-        const double Si = fma(-v, s_min[5 * TZ + row], s_min[4 * TZ + row]);
+        const double Sd = fma(-v, mom(s, 1), mom(s, 0));
+        const double Sr = fma(-v, mom(s, 3), mom(s, 2));
+        const double Si = fma(-v, mom(s, 5), mom(s, 4));
 #pragma unroll
         for (int sp = 0; sp < 2; ++sp) {
           const double A = sp == 0 ? p.A0 + Sd : p.A0 - Sd;
@@ -223,56 +345,64 @@ __global__ void __launch_bounds__(NSEG* VC, 1)
 
       // ---- S4: RK combine and stores
       double out[8];
+      const long long gidx = (iz + G) * p.nvp + j;
 #pragma unroll
       for (int c = 0; c < 8; ++c) {
-        double accb;
+        double u0v = yc[c], accb;
+        if constexpr (KT::LOAD_U0) u0v = lds(Tu + ((c * TZ + row) * VC) * 8);
         if constexpr (KIND == FIRST || KIND == FIRST_LEAN) accb = yc[c];
-        else if constexpr (KIND == MID_REBUILD) accb = fma(yc[c] - u0v[c], 1.0 / 3.0, u0v[c]);  // u0 + (dt/6) k1
-        else accb = accv[c];
-        const double base = (KIND == LAST) ? accb : u0v[c];
-        out[c] = fma(p.cy, k[c], base);
-        if (act) {
+        else if constexpr (KIND == MID_REBUILD) accb = fma(yc[c] - u0v, 1.0 / 3.0, u0v);  // u0 + (dt/6) k1
+        else accb = lds(Ta + ((c * TZ + row) * VC) * 8);
+        const double base = (KIND == LAST) ? accb : u0v;
+        out[c] = act ? fma(p.cy, k[c], base) : 0.0;
+        k[c] = fma(p.ca, k[c], accb);   // new accumulator value
+      }
+      if (act) {
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
           double* yo = p.y_out + c * p.comp_stride + gidx;
           *yo = out[c];
-          if (iz < G) yo[p.nz * p.nvp] = out[c];                 // right ghost copy of the first rows
-          if (iz >= p.nz - G) yo[-p.nz * p.nvp] = out[c];        // left ghost copy of the last rows
-          if constexpr (WRITE_ACC) p.acc_out[c * p.comp_stride + gidx] = fma(p.ca, k[c], accb);
-        } else {
-          out[c] = 0.0;
+          if constexpr (KT::WRITE_ACC) p.acc_out[c * p.comp_stride + gidx] = k[c];
+        }
+        if (iz < G) {                      // right ghost copy of the first rows
+#pragma unroll
+          for (int c = 0; c < 8; ++c) p.y_out[c * p.comp_stride + gidx + p.nz * p.nvp] = out[c];
+        }
+        if (iz >= p.nz - G) {              // left ghost copy of the last rows
+#pragma unroll
+          for (int c = 0; c < 8; ++c) p.y_out[c * p.comp_stride + gidx - p.nz * p.nvp] = out[c];
         }
       }
 
       // ---- S5: velocity moments of the produced state, D = rho - rhobar^*
-      double m[6];
-      m[0] = (out[0] - out[1]) - (out[4] - out[5]);
-      m[2] = out[2] - out[6];
-      m[4] = out[3] + out[7];
-      m[1] = v * m[0];
-      m[3] = v * m[2];
-      m[5] = v * m[4];
-#pragma unroll
-      for (int q = 0; q < 6; ++q) {
-#pragma unroll
-        for (int off = VC / 2; off > 0; off >>= 1) m[q] += __shfl_xor_sync(0xffffffffu, m[q], off);
-      }
-      if (lane == 0 && valid) {
-#pragma unroll
-        for (int q = 0; q < 6; ++q) s_macc[q * TZ + row] += m[q];
-      }
+      mred[6 * s + 0] = (out[0] - out[1]) - (out[4] - out[5]);
+      mred[6 * s + 2] = out[2] - out[6];
+      mred[6 * s + 4] = out[3] + out[7];
+      mred[6 * s + 1] = v * mred[6 * s + 0];
+      mred[6 * s + 3] = v * mred[6 * s + 2];
+      mred[6 * s + 5] = v * mred[6 * s + 4];
     }
 
-    __syncthreads();  // every thread is done with this buffer
-    if (tid == 0 && ch + NBUF < nchunks) {
-      mbar_expect_tx(&full[buf], TILE * 8);
-      tma_load_3d(tile + buf * TILE, &tmap_y, &full[buf], (ch + NBUF) * VC, (int)(iz0 + G - H), 0);
+    // all shared-memory reads of this item are done: hand the slots back to the producer
+    __syncwarp();
+    if (lane == 0) {
+      mbar_arrive(b_empty_y + 8 * sy);
+      if constexpr (NARR > 0) mbar_arrive(b_empty_ua + 8 * (int)(n % NUA));
     }
-  }
 
-  __syncthreads();
-  for (int q = tid; q < 6 * TZ; q += NT) {
-    const int m = q / TZ, r = q - m * TZ;
-    const long long iz = iz0 + r;
-    if (iz < p.nz) p.mom_out[(long long)m * p.nz + iz] = s_macc[q] * p.dv;
+    int midx;
+    bool mvalid;
+    butterfly_reduce<6 * S>(mred, lane, midx, mvalid);
+    macc += mred[0];
+    if (++ch == nchunks) {
+      if (mvalid) {
+        const long long iz = iz0 + row0 + midx / 6;
+        if (iz < p.nz) p.mom_out[(long long)(midx % 6) * p.nz + iz] = macc * p.dv;
+      }
+      macc = 0.0;
+      ch = 0;
+      tile += gridDim.x;
+    }
   }
 }
 

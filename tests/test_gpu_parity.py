@@ -47,29 +47,32 @@ def run_pair(B, R, args, st, nsteps, **opts):
     return got, ref, gm, rm, gd, rd
 
 
-# ---- sizes: several z-tiles (TZ = 32) and v-chunks (VC = 32 / 16), ragged tails in both directions
-SHAPES = [(64, 16), (1024, 16), (100, 8), (77, 3), (96, 40), (250, 100), (129, 130), (16, 2)]
+# ---- sizes: several z-tiles (TZ = 16) and v-chunks (32 beams), ragged tails in both directions,
+# more tiles than SMs (persistent CTAs take several tiles) and fewer
+SHAPES = [(64, 16), (1024, 16), (100, 8), (77, 3), (96, 40), (250, 100), (129, 130), (16, 2), (5000, 33)]
 
 
+@pytest.mark.parametrize("variant", [0, 1])
 @pytest.mark.parametrize("scheme", [FD, FV])
 @pytest.mark.parametrize("nz,nv", SHAPES)
-def test_one_step_random_state(B, R, scheme, nz, nv):
+def test_one_step_random_state(B, R, scheme, nz, nv, variant):
     """One RK4 step from an O(1) random (rough) state: every term of the RHS is exercised at full size."""
     st = inputs.random_state(nz, nv, seed=100 + nz + nv)
     args = (nz, nv, 0.7 * nz, 0.05, 0.8, 0.3, 1.3, scheme)
-    got, ref, gm, rm, _, _ = run_pair(B, R, args, st, 1)
+    got, ref, gm, rm, _, _ = run_pair(B, R, args, st, 1, variant=variant)
     assert np.max(np.abs(got - ref)) <= 2e-14 * max(1.0, np.max(np.abs(ref)))
     assert np.max(np.abs(gm - rm)) <= 1e-14 * max(1.0, np.max(np.abs(rm)))
 
 
+@pytest.mark.parametrize("variant", [0, 1])
 @pytest.mark.parametrize("scheme", [FD, FV])
 @pytest.mark.parametrize("lean", [False, True])
-def test_20_steps_cfg0_shape(B, R, scheme, lean):
+def test_20_steps_cfg0_shape(B, R, scheme, lean, variant):
     """BASELINE config 0 (fast conversion, 1024 x 16, dt = 0.4 dz), 20 steps, both schemes."""
     c = inputs.CONFIGS["cfg0"]
     st = inputs.config_state("cfg0")
     args = (c["nz"], c["nv"], c["L"], c["dt"], c["omega"], c["theta"], c["mu"], scheme)
-    got, ref, gm, rm, gd, rd = run_pair(B, R, args, st, 20, lean_acc=lean)
+    got, ref, gm, rm, gd, rd = run_pair(B, R, args, st, 20, lean_acc=lean, variant=variant)
     assert np.max(np.abs(got - ref)) <= TOL20
     assert np.max(np.abs(gm - rm)) <= TOL20
     assert abs(gd["psurv_nu"] - rd["psurv_nu"]) <= 1e-12
