@@ -4,7 +4,14 @@
 
 extern "C" double cosenu_probe_weno7_face(const double* w7, double v, double eps) {
   // value of f = v u at the interface, as the kernels form it
-  return v * cosenu_math::weno7_face(w7, v * v, eps);
+  return v * cosenu_math::weno7_face(w7, cosenu_math::weno7_beam(v, eps));
+}
+
+// two adjacent interfaces from 8 cells (shared differences): out[0] = w[3]|w[4], out[1] = w[4]|w[5]
+extern "C" void cosenu_probe_weno7_face2(const double* w8, double v, double eps, double* out) {
+  double a, b;
+  cosenu_math::weno7_face2(w8, cosenu_math::weno7_beam(v, eps), a, b);
+  out[0] = v * a; out[1] = v * b;
 }
 
 extern "C" double cosenu_probe_fd4_ko3(const double* u5, double v, double dz, double eps_ko) {

@@ -73,6 +73,23 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "r"(parity)
       : "memory");
 }
+// the producer's wait: back off between probes so that the spin does not take issue slots from the compute warps
+__device__ __forceinline__ void mbar_wait_backoff(uint32_t bar, uint32_t parity) {
+  uint32_t done = 0;
+  while (true) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(done)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    if (done) break;
+    __nanosleep(128);
+  }
+}
 // 3-D tiled TMA load global -> shared, completion on an mbarrier
 __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1, int c2) {
   asm volatile(
@@ -151,6 +168,54 @@ __device__ __forceinline__ void butterfly_reduce(double (&x)[N], int lane, int& 
   idx = pos;
 }
 
+// ----------------------------------------------------------------------------- WENO7 fluxes of a warp's rows
+// Tw = shared address of (component 0, tile row 0 [halo included], this lane) of the stage-input tile plus
+// rel_row*256: every load below then has an immediate offset.  DIR = +1 for v >= 0 (stencil biased to
+// smaller z), -1 for v < 0 (mirror image about the interface, reading A9).
+// FR[s][c] = WENO7 value of u_c at the right interface of row (rel_row + s).
+template <int DIR, int S, int ROWS, int H>
+__device__ __forceinline__ void weno_rows(uint32_t Tw, const cosenu_math::Weno7Beam& bm, double (&FR)[S][8]) {
+  static_assert(S == 1 || S == 2, "rows per warp");
+#pragma unroll
+  for (int c = 0; c < 8; ++c) {
+    if constexpr (S == 1) {
+      double w[7];
+#pragma unroll
+      for (int k = 0; k < 7; ++k) w[k] = lds(Tw + ((c * ROWS + H + (DIR > 0 ? 0 : 1) + DIR * (k - 3)) * VC) * 8);
+      FR[0][c] = cosenu_math::weno7_face(w, bm);
+    } else {
+      double w[8], Fa, Fb;
+#pragma unroll
+      for (int k = 0; k < 8; ++k) w[k] = lds(Tw + ((c * ROWS + H + (DIR > 0 ? k - 3 : 5 - k)) * VC) * 8);
+      cosenu_math::weno7_face2(w, bm, Fa, Fb);
+      FR[DIR > 0 ? 0 : 1][c] = Fa;
+      FR[DIR > 0 ? 1 : 0][c] = Fb;
+    }
+  }
+}
+// value at the left boundary interface of the tile (between tile rows H-1 and H) of one component
+template <int DIR, int ROWS, int H>
+__device__ __forceinline__ double weno_boundary(uint32_t Tc /* component base + lane */, const cosenu_math::Weno7Beam& bm) {
+  double w[7];
+#pragma unroll
+  for (int k = 0; k < 7; ++k) w[k] = lds(Tc + ((H - 1 + (DIR > 0 ? 0 : 1) + DIR * (k - 3)) * VC) * 8);
+  return cosenu_math::weno7_face(w, bm);
+}
+// out-of-line copies for warps whose lanes move in both directions (only the chunk that contains v = 0)
+template <int DIR, int S, int ROWS, int H>
+__device__ __noinline__ void weno_rows_slow(uint32_t Tw, const cosenu_math::Weno7Beam& bm, double* FRflat) {
+  double FR[S][8];
+  weno_rows<DIR, S, ROWS, H>(Tw, bm, FR);
+#pragma unroll
+  for (int s = 0; s < S; ++s)
+#pragma unroll
+    for (int c = 0; c < 8; ++c) FRflat[s * 8 + c] = FR[s][c];
+}
+template <int DIR, int ROWS, int H>
+__device__ __noinline__ double weno_boundary_slow(uint32_t Tc, const cosenu_math::Weno7Beam& bm) {
+  return weno_boundary<DIR, ROWS, H>(Tc, bm);
+}
+
 // ----------------------------------------------------------------------------- the stage kernel
 template <int SCHEME, int KIND, int TZ, int NSEG, int NY, int NUA>
 __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
@@ -196,12 +261,12 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
       for (long long n = 0; n < nitems; ++n) {
         const int iz0 = (int)(tile * TZ);
         const int sy = (int)(n % NY);
-        mbar_wait(b_empty_y + 8 * sy, (uint32_t)(((n / NY) & 1) ^ 1));
+        mbar_wait_backoff(b_empty_y + 8 * sy, (uint32_t)(((n / NY) & 1) ^ 1));
         mbar_expect_tx(b_full_y + 8 * sy, SM::YTILE);
         tma_load_3d(s_y + sy * SM::YTILE, &tm_y, b_full_y + 8 * sy, ch * VC, iz0 + G - H, 0);
         if constexpr (NARR > 0) {
           const int su = (int)(n % NUA);
-          mbar_wait(b_empty_ua + 8 * su, (uint32_t)(((n / NUA) & 1) ^ 1));
+          mbar_wait_backoff(b_empty_ua + 8 * su, (uint32_t)(((n / NUA) & 1) ^ 1));
           mbar_expect_tx(b_full_ua + 8 * su, NARR * SM::PTILE);
           uint32_t dst = s_ua + su * NARR * SM::PTILE;
           if constexpr (KT::LOAD_U0) { tma_load_3d(dst, &tm_u0, b_full_ua + 8 * su, ch * VC, iz0 + G, 0); dst += SM::PTILE; }
@@ -216,17 +281,24 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
   // =========================================================================== compute warps
   const int row0 = warp * S;
   double macc = 0.0;      // running moment (one (row, quantity) per valid lane, see butterfly_reduce)
-  double min_cur = 0.0;   // lane l < 6S: mu * moment (l % 6) of row row0 + l / 6 of the stage input
+  // lane l < 6S holds mu * moment (l % 6) of row row0 + l / 6 of the stage input; the next tile's values are
+  // fetched one tile ahead so that their latency is never exposed
+  auto load_min = [&](long long t) {
+    double m = 0.0;
+    if (lane < 6 * S && t < ntiles) {
+      const long long iz = t * TZ + row0 + lane / 6;
+      if (iz < p.nz) m = p.mu * __ldg(p.mom_in + (long long)(lane % 6) * p.nz + iz);
+    }
+    return m;
+  };
+  double min_cur = 0.0, min_next = load_min(blockIdx.x);
   long long tile = blockIdx.x;
   int ch = 0;
   for (long long n = 0; n < nitems; ++n) {
     const long long iz0 = tile * TZ;
     if (ch == 0) {
-      min_cur = 0.0;
-      if (lane < 6 * S) {
-        const long long iz = iz0 + row0 + lane / 6;
-        if (iz < p.nz) min_cur = p.mu * __ldg(p.mom_in + (long long)(lane % 6) * p.nz + iz);
-      }
+      min_cur = min_next;
+      min_next = load_min(tile + gridDim.x);
     }
     const int sy = (int)(n % NY);
     const uint32_t Ty = s_y + sy * SM::YTILE + lane * 8;   // + ((c * ROWS + r) * 32) * 8
@@ -241,29 +313,30 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
     double FL[8];
     double nvz = 0.0, cadv_v = 0.0;
     if constexpr (SCHEME == 1) {
-      const int wdir = v >= 0.0 ? 1 : -1;
-      const int rsh = wdir > 0 ? 0 : 1;       // centre cell of the upwind-biased stencil: i or i+1
-      const int wstep = wdir * VC * 8;        // byte step of one stencil cell towards the downwind side
-      const double v2 = v * v;
       nvz = v * p.ninv_dz;
-#pragma unroll
-      for (int s = 0; s < S; ++s) {
-#pragma unroll
-        for (int c = 0; c < 8; ++c) {
-          const uint32_t b = Ty + ((c * ROWS + row0 + s + H + rsh) * VC) * 8;
-          double w[7];
-#pragma unroll
-          for (int k = 0; k < 7; ++k) w[k] = lds(b + (k - 3) * wstep);
-          FR[s][c] = cosenu_math::weno7_face(w, v2, p.weno_eps);
-        }
-      }
+      const cosenu_math::Weno7Beam bm = cosenu_math::weno7_beam(v, p.weno_eps);
+      const uint32_t Tw = Ty + row0 * (VC * 8);
+      const uint32_t Tc = Ty + (warp & 7) * (ROWS * VC * 8);   // boundary piece: component `warp` (warps 0..7)
+      const unsigned mpos = __ballot_sync(0xffffffffu, v >= 0.0);
       double FB = 0.0;
-      if (warp < 8) {  // left boundary interface of the tile, component `warp`
-        const uint32_t b = Ty + ((warp * ROWS + H - 1 + rsh) * VC) * 8;
-        double w[7];
+      if (mpos == 0xffffffffu) {
+        weno_rows<1, S, ROWS, H>(Tw, bm, FR);
+        if (warp < 8) FB = weno_boundary<1, ROWS, H>(Tc, bm);
+      } else if (mpos == 0u) {
+        weno_rows<-1, S, ROWS, H>(Tw, bm, FR);
+        if (warp < 8) FB = weno_boundary<-1, ROWS, H>(Tc, bm);
+      } else {
+        double Fp[S * 8], Fm[S * 8];
+        weno_rows_slow<1, S, ROWS, H>(Tw, bm, Fp);
+        weno_rows_slow<-1, S, ROWS, H>(Tw, bm, Fm);
 #pragma unroll
-        for (int k = 0; k < 7; ++k) w[k] = lds(b + (k - 3) * wstep);
-        FB = cosenu_math::weno7_face(w, v2, p.weno_eps);
+        for (int s = 0; s < S; ++s)
+#pragma unroll
+          for (int c = 0; c < 8; ++c) FR[s][c] = v >= 0.0 ? Fp[s * 8 + c] : Fm[s * 8 + c];
+        if (warp < 8) {
+          const double bp = weno_boundary_slow<1, ROWS, H>(Tc, bm), bn = weno_boundary_slow<-1, ROWS, H>(Tc, bm);
+          FB = v >= 0.0 ? bp : bn;
+        }
       }
       mbar_wait(b_xfree, (uint32_t)((n & 1) ^ 1));   // readers of the previous item are done
 #pragma unroll

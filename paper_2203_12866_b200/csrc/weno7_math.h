@@ -25,10 +25,14 @@
 // d_0..d_3 = 4/35, 18/35, 12/35, 1/35 reproduces Eq. (A.1), reading A6).
 //
 // The reconstruction acts on f = v u with v constant along z (reading A8), so
-// SI_r[f] = v^2 SI_r[u] and  fhat[f] = v fhat[u]:  the routine works on u and takes v^2.
-// The nonlinear weights  w_r = d_r / (SI_r + eps)^2  (Eq. 14) are combined with ONE division:
-//      F = sum_r w_r fhat_r / sum_r w_r = u_i + (1/2) [sum_r W_r (A_r + s_r/6)] / [sum_r W_r],
-//      W_r = d_r prod_{m != r} (SI_m + eps)^2.
+// SI_r[f] = v^2 SI_r[u] and  fhat[f] = v fhat[u]:  the routines work on u.
+// The nonlinear weights  w_r = d_r / (SI_r + eps)^2  (Eq. 14) are combined with ONE division.  With
+//      qs_r = (SI_r[u] + eps/v^2) / sqrt(d_r)        (so that  w_r  is proportional to  1 / qs_r^2),
+//      P_r  = prod_{m != r} qs_m^2,
+//      F = sum_r w_r fhat_r / sum_r w_r = u_i + (1/2) [sum_r P_r (A_r + s_r/6)] / [sum_r P_r].
+// The per-beam constants  eps_r = (eps/v^2)/sqrt(d_r)  are formed once per beam (Weno7Beam).
+// Range: needs |u|^2 * 1e4 / v^2-scaled terms to stay below ~1e50 per factor (states are O(1)); v^2 is
+// clamped to >= 1e-40 (the flux is multiplied by v afterwards, so v = 0 gives exactly 0).
 #ifndef COSENU_WENO7_MATH_H
 #define COSENU_WENO7_MATH_H
 
@@ -42,14 +46,12 @@ using std::fma;
 
 namespace cosenu_math {
 
-// reciprocal to ~1 ulp: hardware seed + 2 Newton steps on the device, plain division on the host
-COSENU_HD double fast_rcp(double d) {
+// reciprocal: hardware seed (MUFU.RCP64H) + 2 Newton steps on the device (~1 ulp), plain division on the host
+COSENU_HD double fast_rcp2(double d) {
 #ifdef __CUDA_ARCH__
   double x;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(d));
   double e = fma(-d, x, 1.0);
-  x = fma(x, e, x);
-  e = fma(-d, x, 1.0);
   x = fma(x, e, x);
   e = fma(-d, x, 1.0);
   x = fma(x, e, x);
@@ -59,35 +61,69 @@ COSENU_HD double fast_rcp(double d) {
 #endif
 }
 
-// WENO7 value of u at the interface between w[3] and w[4], biased towards w[0] (the upwind side):
-// w[0..6] = u_{i-3} .. u_{i+3} for v >= 0; the mirrored cells u_{i+4} .. u_{i-2} for v < 0.
-// v2 = v^2, eps = epsilon of Eq. (14).
-COSENU_HD double weno7_face(const double w[7], double v2, double eps) {
-  const double D0 = w[1] - w[0], D1 = w[2] - w[1], D2 = w[3] - w[2], D3 = w[4] - w[3], D4 = w[5] - w[4],
-               D5 = w[6] - w[5];
-  const double E0 = D1 - D0, E1 = D2 - D1, E2 = D3 - D2, E3 = D4 - D3, E4 = D5 - D4;
-  const double T0 = E1 - E0, T1 = E2 - E1, T2 = E3 - E2, T3 = E4 - E3;
-  // A_r, s_r per sub-stencil (x, p, q, t) = (D[3-r], E[3-r], E[4-r], T[3-r])
+// per-beam constants of the weights: eps_r = (eps / v^2) / sqrt(d_r), d = (4, 18, 12, 1)/35
+struct Weno7Beam {
+  double e0, e1, e2, e3;
+};
+COSENU_HD Weno7Beam weno7_beam(double v, double eps) {
+  double v2 = v * v;
+  if (v2 < 1e-40) v2 = 1e-40;
+  const double ev = eps / v2;
+  Weno7Beam b;
+  b.e0 = ev * 2.9580398915498080213;   // sqrt(35/4)
+  b.e1 = ev * 1.3944333775567926;      // sqrt(35/18)
+  b.e2 = ev * 1.7078251276599330;      // sqrt(35/12)
+  b.e3 = ev * 5.9160797830996160426;   // sqrt(35)
+  return b;
+}
+
+// the part of Algorithm 1 after the undivided differences: D[0..5], E[0..4], T[0..3] of the 7 cells
+// w[0..6] (D_k = w[k+1]-w[k], E_k = D[k+1]-D[k], T_k = E[k+1]-E[k]); ui = w[3].
+COSENU_HD double weno7_core(double ui, double D0, double D1, double D2, double D3, double E0, double E1, double E2,
+                            double E3, double E4, double T0, double T1, double T2, double T3, const Weno7Beam& bm) {
+  // A_r, s_r per sub-stencil: (x, p, q, t) = (D[3-r], E[3-r], E[4-r], T[3-r])
   const double A0 = fma(1.0 / 3.0, E4, fma(-5.0 / 6.0, E3, D3));
   const double A1 = fma(-1.0 / 6.0, E3, fma(2.0 / 3.0, E2, D2));
   const double A2 = fma(1.0 / 3.0, E2, fma(7.0 / 6.0, E1, D1));
   const double A3 = fma(11.0 / 6.0, E1, fma(2.0 / 3.0, E0, D0));
-  const double s0 = E3 - T3, s1 = E2, s2 = E2, s3 = E1 + T0;
-  const double ca = 240.0 * v2, cs = 260.0 * v2, ct = (781.0 / 3.0) * v2;
-  // q_r = v^2 SI_r[u] + eps
-  const double q0 = fma(ca, A0 * A0, fma(cs, s0 * s0, fma(ct, T3 * T3, eps)));
-  const double q1 = fma(ca, A1 * A1, fma(cs, s1 * s1, fma(ct, T2 * T2, eps)));
-  const double q2 = fma(ca, A2 * A2, fma(cs, s2 * s2, fma(ct, T1 * T1, eps)));
-  const double q3 = fma(ca, A3 * A3, fma(cs, s3 * s3, fma(ct, T0 * T0, eps)));
+  const double s0 = E3 - T3, s3 = E1 + T0;   // s1 = s2 = E2
+  const double ss12 = E2 * E2;
+  // qs_r = (240 A^2 + 260 s^2 + (781/3) t^2 + eps/v^2) / sqrt(d_r)
+  constexpr double k0 = 2.9580398915498080213, k1 = 1.3944333775567926, k2 = 1.7078251276599330,
+                   k3 = 5.9160797830996160426;
+  const double q0 = fma(240.0 * k0, A0 * A0, fma(260.0 * k0, s0 * s0, fma((781.0 / 3.0) * k0, T3 * T3, bm.e0)));
+  const double q1 = fma(240.0 * k1, A1 * A1, fma(260.0 * k1, ss12, fma((781.0 / 3.0) * k1, T2 * T2, bm.e1)));
+  const double q2 = fma(240.0 * k2, A2 * A2, fma(260.0 * k2, ss12, fma((781.0 / 3.0) * k2, T1 * T1, bm.e2)));
+  const double q3 = fma(240.0 * k3, A3 * A3, fma(260.0 * k3, s3 * s3, fma((781.0 / 3.0) * k3, T0 * T0, bm.e3)));
   const double Q0 = q0 * q0, Q1 = q1 * q1, Q2 = q2 * q2, Q3 = q3 * q3;
   const double Q01 = Q0 * Q1, Q23 = Q2 * Q3;
-  const double W0 = (4.0 / 35.0) * (Q1 * Q23), W1 = (18.0 / 35.0) * (Q0 * Q23);
-  const double W2 = (12.0 / 35.0) * (Q01 * Q3), W3 = (1.0 / 35.0) * (Q01 * Q2);
-  const double den = (W0 + W1) + (W2 + W3);
-  const double c0 = fma(1.0 / 6.0, s0, A0), c1 = fma(1.0 / 6.0, s1, A1), c2 = fma(1.0 / 6.0, s2, A2),
+  const double P0 = Q1 * Q23, P1 = Q0 * Q23, P2 = Q01 * Q3, P3 = Q01 * Q2;
+  const double den = (P0 + P1) + (P2 + P3);
+  const double c0 = fma(1.0 / 6.0, s0, A0), c1 = fma(1.0 / 6.0, E2, A1), c2 = fma(1.0 / 6.0, E2, A2),
                c3 = fma(1.0 / 6.0, s3, A3);
-  const double num = fma(W0, c0, fma(W1, c1, fma(W2, c2, W3 * c3)));
-  return fma(num, 0.5 * fast_rcp(den), w[3]);
+  const double num = fma(P0, c0, fma(P1, c1, fma(P2, c2, P3 * c3)));
+  return fma(num, 0.5 * fast_rcp2(den), ui);
+}
+
+// WENO7 value of u at the interface between w[3] and w[4], biased towards w[0] (the upwind side):
+// w[0..6] = u_{i-3} .. u_{i+3} for v >= 0; the mirrored cells u_{i+4} .. u_{i-2} for v < 0.
+COSENU_HD double weno7_face(const double w[7], const Weno7Beam& bm) {
+  const double D0 = w[1] - w[0], D1 = w[2] - w[1], D2 = w[3] - w[2], D3 = w[4] - w[3], D4 = w[5] - w[4],
+               D5 = w[6] - w[5];
+  const double E0 = D1 - D0, E1 = D2 - D1, E2 = D3 - D2, E3 = D4 - D3, E4 = D5 - D4;
+  const double T0 = E1 - E0, T1 = E2 - E1, T2 = E3 - E2, T3 = E4 - E3;
+  return weno7_core(w[3], D0, D1, D2, D3, E0, E1, E2, E3, E4, T0, T1, T2, T3, bm);
+}
+
+// two adjacent interfaces from 8 cells w[0..7] with shared differences:
+//   Fa = interface between w[3] and w[4],  Fb = interface between w[4] and w[5], both biased towards w[0].
+COSENU_HD void weno7_face2(const double w[8], const Weno7Beam& bm, double& Fa, double& Fb) {
+  const double D0 = w[1] - w[0], D1 = w[2] - w[1], D2 = w[3] - w[2], D3 = w[4] - w[3], D4 = w[5] - w[4],
+               D5 = w[6] - w[5], D6 = w[7] - w[6];
+  const double E0 = D1 - D0, E1 = D2 - D1, E2 = D3 - D2, E3 = D4 - D3, E4 = D5 - D4, E5 = D6 - D5;
+  const double T0 = E1 - E0, T1 = E2 - E1, T2 = E3 - E2, T3 = E4 - E3, T4 = E5 - E4;
+  Fa = weno7_core(w[3], D0, D1, D2, D3, E0, E1, E2, E3, E4, T0, T1, T2, T3, bm);
+  Fb = weno7_core(w[4], D1, D2, D3, D4, E1, E2, E3, E4, E5, T1, T2, T3, T4, bm);
 }
 
 // FD4 + KO3 in difference form (Eq. (5)): returns
