@@ -53,7 +53,7 @@ struct cosenu {
   int64_t comp_stride = 0; size_t state_elems = 0;
   int mcur = 0;  // M[mcur] holds the moments of U
   CUtensorMap tm_U, tm_Y1, tm_Y2;   // stage-input boxes [8][TZ+2H][32]
-  CUtensorMap tp_U, tp_ACC;         // plain boxes [8][TZ][32] (u0, RK accumulator)
+  CUtensorMap tp_U, tp_Y1, tp_Y2, tp_ACC;   // rows 0..nz-1 only, boxes [8][TZ][32]: u0 / acc loads, output stores
   bool maps_ready = false;
 
   bool have_state = false;
@@ -103,8 +103,11 @@ size_t workspace_layout(const cosenu* h, size_t off[10]) {
   return o;
 }
 
-int make_map(cosenu* h, PFN_encodeTiled enc, CUtensorMap* map, double* base, int rows_box) {
-  const cuuint64_t gdim[3] = {(cuuint64_t)h->nv, (cuuint64_t)(h->nz + 2 * G), 8};
+// with_ghosts: the view covers device rows 0..nz+2G-1 (stencil input); otherwise rows G..G+nz-1 (z = 0..nz-1),
+// so that out-of-range rows of a ragged last tile are clipped by the TMA store instead of hitting ghost rows
+int make_map(cosenu* h, PFN_encodeTiled enc, CUtensorMap* map, double* base, int rows_box, bool with_ghosts) {
+  if (!with_ghosts) base += (size_t)G * h->nvp;
+  const cuuint64_t gdim[3] = {(cuuint64_t)h->nv, (cuuint64_t)(with_ghosts ? h->nz + 2 * G : h->nz), 8};
   const cuuint64_t gstr[2] = {(cuuint64_t)h->nvp * 8, (cuuint64_t)h->comp_stride * 8};
   const cuuint32_t box[3] = {(cuuint32_t)VC, (cuuint32_t)rows_box, 8};
   const cuuint32_t estr[3] = {1, 1, 1};
@@ -139,17 +142,19 @@ int ensure_workspace(cosenu* h) {
   PFN_encodeTiled enc = reinterpret_cast<PFN_encodeTiled>(fn);
   const int rows = TZ_ALL + 2 * (h->scheme == COSENU_FD4_KO3 ? 2 : 4);
   int rc;
-  if ((rc = make_map(h, enc, &h->tm_U, h->U, rows))) return rc;
-  if ((rc = make_map(h, enc, &h->tm_Y1, h->Y1, rows))) return rc;
-  if ((rc = make_map(h, enc, &h->tm_Y2, h->Y2, rows))) return rc;
-  if ((rc = make_map(h, enc, &h->tp_U, h->U, TZ_ALL))) return rc;
-  if ((rc = make_map(h, enc, &h->tp_ACC, h->ACC, TZ_ALL))) return rc;
+  if ((rc = make_map(h, enc, &h->tm_U, h->U, rows, true))) return rc;
+  if ((rc = make_map(h, enc, &h->tm_Y1, h->Y1, rows, true))) return rc;
+  if ((rc = make_map(h, enc, &h->tm_Y2, h->Y2, rows, true))) return rc;
+  if ((rc = make_map(h, enc, &h->tp_U, h->U, TZ_ALL, false))) return rc;
+  if ((rc = make_map(h, enc, &h->tp_Y1, h->Y1, TZ_ALL, false))) return rc;
+  if ((rc = make_map(h, enc, &h->tp_Y2, h->Y2, TZ_ALL, false))) return rc;
+  if ((rc = make_map(h, enc, &h->tp_ACC, h->ACC, TZ_ALL, false))) return rc;
   h->maps_ready = true;
   return COSENU_OK;
 }
 
 template <int SCHEME, int KIND, int TZ, int NSEG, int NY, int NUA>
-int launch_one(cosenu* h, const CUtensorMap& map, const StageParams& p) {
+int launch_one(cosenu* h, const CUtensorMap& map, const CUtensorMap& omap, const StageParams& p) {
   auto kern = stage_kernel<SCHEME, KIND, TZ, NSEG, NY, NUA>;
   constexpr size_t smem = StageSmem<SCHEME, KIND, TZ, NSEG, NY, NUA>::bytes;
   static_assert(smem <= 232448, "over the 227 KB shared-memory limit of a CTA");
@@ -160,30 +165,30 @@ int launch_one(cosenu* h, const CUtensorMap& map, const StageParams& p) {
   }
   const long long ntiles = (h->nz + TZ - 1) / TZ;
   const unsigned grid = (unsigned)(ntiles < h->num_sms ? ntiles : h->num_sms);   // persistent: one CTA per SM
-  kern<<<grid, NSEG * 32 + 32, smem, h->stream>>>(map, h->tp_U, h->tp_ACC, p);
+  kern<<<grid, NSEG * 32 + 32, smem, h->stream>>>(map, h->tp_U, h->tp_ACC, omap, p);
   CK(cudaGetLastError());
   h->launches++;
   return COSENU_OK;
 }
 
 template <int SCHEME, int TZ, int NSEG, int NY, int NUA>
-int launch_kind(cosenu* h, int kind, const CUtensorMap& map, const StageParams& p) {
+int launch_kind(cosenu* h, int kind, const CUtensorMap& map, const CUtensorMap& omap, const StageParams& p) {
   switch (kind) {
-    case FIRST: return launch_one<SCHEME, FIRST, TZ, NSEG, NY, NUA>(h, map, p);
-    case FIRST_LEAN: return launch_one<SCHEME, FIRST_LEAN, TZ, NSEG, NY, NUA>(h, map, p);
-    case MID: return launch_one<SCHEME, MID, TZ, NSEG, NY, NUA>(h, map, p);
-    case MID_REBUILD: return launch_one<SCHEME, MID_REBUILD, TZ, NSEG, NY, NUA>(h, map, p);
-    default: return launch_one<SCHEME, LAST, TZ, NSEG, NY, NUA>(h, map, p);
+    case FIRST: return launch_one<SCHEME, FIRST, TZ, NSEG, NY, NUA>(h, map, omap, p);
+    case FIRST_LEAN: return launch_one<SCHEME, FIRST_LEAN, TZ, NSEG, NY, NUA>(h, map, omap, p);
+    case MID: return launch_one<SCHEME, MID, TZ, NSEG, NY, NUA>(h, map, omap, p);
+    case MID_REBUILD: return launch_one<SCHEME, MID_REBUILD, TZ, NSEG, NY, NUA>(h, map, omap, p);
+    default: return launch_one<SCHEME, LAST, TZ, NSEG, NY, NUA>(h, map, omap, p);
   }
 }
 
-int launch_stage(cosenu* h, int kind, const CUtensorMap& map, const StageParams& p) {
+int launch_stage(cosenu* h, int kind, const CUtensorMap& map, const CUtensorMap& omap, const StageParams& p) {
   if (h->scheme == COSENU_FD4_KO3) {
-    if (h->variant == 1) return launch_kind<0, TZ_ALL, 8, 2, 2>(h, kind, map, p);
-    return launch_kind<0, TZ_ALL, 16, 2, 2>(h, kind, map, p);
+    if (h->variant == 1) return launch_kind<0, TZ_ALL, 8, 2, 2>(h, kind, map, omap, p);
+    return launch_kind<0, TZ_ALL, 16, 2, 2>(h, kind, map, omap, p);
   }
-  if (h->variant == 1) return launch_kind<1, TZ_ALL, 8, 2, 1>(h, kind, map, p);
-  return launch_kind<1, TZ_ALL, 16, 2, 1>(h, kind, map, p);
+  if (h->variant == 1) return launch_kind<1, TZ_ALL, 8, 2, 1>(h, kind, map, omap, p);
+  return launch_kind<1, TZ_ALL, 16, 2, 1>(h, kind, map, omap, p);
 }
 
 StageParams base_params(const cosenu* h) {
@@ -243,22 +248,22 @@ int one_step(cosenu* h) {
   // stage 1: k1 = RHS(U); Y1 = U + dt/2 k1; ACC = U + dt/6 k1
   p.y_out = h->Y1; p.acc_out = h->ACC; p.mom_in = Min; p.mom_out = Mout;
   p.cy = 0.5 * dt; p.ca = dt / 6.0;
-  if ((rc = launch_stage(h, h->lean_acc ? FIRST_LEAN : FIRST, h->tm_U, p))) return rc;
+  if ((rc = launch_stage(h, h->lean_acc ? FIRST_LEAN : FIRST, h->tm_U, h->tp_Y1, p))) return rc;
   if (tm) CK(cudaEventRecord(ev[1], h->stream));
   // stage 2: k2 = RHS(Y1); Y2 = U + dt/2 k2; ACC += dt/3 k2
   p.y_out = h->Y2; p.acc_out = h->ACC; p.mom_in = Mout; p.mom_out = Min;
   p.cy = 0.5 * dt; p.ca = dt / 3.0;
-  if ((rc = launch_stage(h, h->lean_acc ? MID_REBUILD : MID, h->tm_Y1, p))) return rc;
+  if ((rc = launch_stage(h, h->lean_acc ? MID_REBUILD : MID, h->tm_Y1, h->tp_Y2, p))) return rc;
   if (tm) CK(cudaEventRecord(ev[2], h->stream));
   // stage 3: k3 = RHS(Y2); Y1 = U + dt k3; ACC += dt/3 k3
   p.y_out = h->Y1; p.mom_in = Min; p.mom_out = Mout;
   p.cy = dt; p.ca = dt / 3.0;
-  if ((rc = launch_stage(h, MID, h->tm_Y2, p))) return rc;
+  if ((rc = launch_stage(h, MID, h->tm_Y2, h->tp_Y1, p))) return rc;
   if (tm) CK(cudaEventRecord(ev[3], h->stream));
   // stage 4: k4 = RHS(Y1); U = ACC + dt/6 k4
   p.y_out = h->U; p.acc_out = nullptr; p.mom_in = Mout; p.mom_out = Min;
   p.cy = dt / 6.0; p.ca = 0.0;
-  if ((rc = launch_stage(h, LAST, h->tm_Y1, p))) return rc;
+  if ((rc = launch_stage(h, LAST, h->tm_Y1, h->tp_U, p))) return rc;
   if (tm) CK(cudaEventRecord(ev[4], h->stream));
   // moments of the new U are in Min = M[mcur] again
   h->t += dt; h->step += 1;

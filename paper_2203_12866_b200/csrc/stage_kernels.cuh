@@ -97,6 +97,17 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map
       "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2)
       : "memory");
 }
+// 3-D tiled TMA store shared -> global (bulk async-group completion); out-of-range elements are clipped
+__device__ __forceinline__ void tma_store_3d(const CUtensorMap* map, uint32_t src, int c0, int c1, int c2) {
+  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];" ::"l"(map), "r"(src),
+               "r"(c0), "r"(c1), "r"(c2)
+               : "memory");
+}
+__device__ __forceinline__ void tma_store_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void tma_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void tma_store_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+// make this thread's shared-memory writes visible to the async proxy (TMA) before signalling
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ double lds(uint32_t addr) {
   double v;
   asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
@@ -111,7 +122,11 @@ struct KindTraits {
   static constexpr bool LOAD_U0 = (KIND == MID || KIND == MID_REBUILD);
   static constexpr bool LOAD_ACC = (KIND == MID || KIND == LAST);
   static constexpr bool WRITE_ACC = (KIND == FIRST || KIND == MID || KIND == MID_REBUILD);
-  static constexpr int NARR = (LOAD_U0 ? 1 : 0) + (LOAD_ACC ? 1 : 0);
+  static constexpr int NLOAD = (LOAD_U0 ? 1 : 0) + (LOAD_ACC ? 1 : 0);
+  // staging arrays of one u0/acc slot: array 0 = u0 on load (acc for LAST), y_out on store;
+  //                                    array 1 = acc on load (MID), acc_out on store
+  static constexpr int NARR = WRITE_ACC ? 2 : 1;
+  static constexpr int ACC_LOAD_ARR = LOAD_U0 ? 1 : 0;
 };
 
 // shared-memory carve-up (byte offsets from a 128-byte aligned base)
@@ -120,7 +135,7 @@ struct StageSmem {
   static constexpr int H = SCHEME == 0 ? 2 : 4;
   static constexpr int ROWS = TZ + 2 * H;
   static constexpr uint32_t YTILE = 8u * ROWS * VC * 8u;   // bytes per stage-input slot
-  static constexpr uint32_t PTILE = 8u * TZ * VC * 8u;     // bytes per u0 / acc slot
+  static constexpr uint32_t PTILE = 8u * TZ * VC * 8u;     // bytes per staging array
   static constexpr int NARR = KindTraits<KIND>::NARR;
   static constexpr uint32_t off_y = 0;
   static constexpr uint32_t off_ua = off_y + NY * YTILE;               // [NUA][NARR][PTILE]
@@ -219,8 +234,11 @@ __device__ __noinline__ double weno_boundary_slow(uint32_t Tc, const cosenu_math
 // ----------------------------------------------------------------------------- the stage kernel
 template <int SCHEME, int KIND, int TZ, int NSEG, int NY, int NUA>
 __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
-    stage_kernel(const __grid_constant__ CUtensorMap tm_y, const __grid_constant__ CUtensorMap tm_u0,
-                 const __grid_constant__ CUtensorMap tm_acc, const StageParams p) {
+    stage_kernel(const __grid_constant__ CUtensorMap tm_y,     // stage input with halo: box [8][TZ+2H][32]
+                 const __grid_constant__ CUtensorMap tm_u0,    // U, rows 0..nz-1: box [8][TZ][32]
+                 const __grid_constant__ CUtensorMap tm_acc,   // RK accumulator (loaded and stored)
+                 const __grid_constant__ CUtensorMap tm_out,   // y_out, rows 0..nz-1
+                 const StageParams p) {
   using SM = StageSmem<SCHEME, KIND, TZ, NSEG, NY, NUA>;
   using KT = KindTraits<KIND>;
   constexpr int H = SM::H, ROWS = SM::ROWS;
@@ -234,9 +252,9 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
   const uint32_t sbase = (smem_u32(smem_raw) + 127u) & ~127u;
   const uint32_t s_y = sbase + SM::off_y, s_ua = sbase + SM::off_ua, s_x = sbase + SM::off_x, s_xb = sbase + SM::off_xb;
   const uint32_t s_bar = sbase + SM::off_bar;
-  // barriers: full_y[NY], empty_y[NY], full_ua[NUA], empty_ua[NUA], xfull, xfree
+  // barriers: full_y[NY], empty_y[NY], full_ua[NUA], out_ready[NUA], xfull, xfree
   const uint32_t b_full_y = s_bar, b_empty_y = s_bar + 8 * NY, b_full_ua = s_bar + 16 * NY,
-                 b_empty_ua = s_bar + 16 * NY + 8 * NUA, b_xfull = s_bar + 16 * NY + 16 * NUA, b_xfree = b_xfull + 8;
+                 b_out_ready = s_bar + 16 * NY + 8 * NUA, b_xfull = s_bar + 16 * NY + 16 * NUA, b_xfree = b_xfull + 8;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int nchunks = (p.nv + VC - 1) / VC;
@@ -246,16 +264,29 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
 
   if (threadIdx.x == 0) {
     for (int b = 0; b < NY; ++b) { mbar_init(b_full_y + 8 * b, 1); mbar_init(b_empty_y + 8 * b, NW); }
-    for (int b = 0; b < NUA; ++b) { mbar_init(b_full_ua + 8 * b, 1); mbar_init(b_empty_ua + 8 * b, NW); }
+    for (int b = 0; b < NUA; ++b) { mbar_init(b_full_ua + 8 * b, 1); mbar_init(b_out_ready + 8 * b, NW); }
     mbar_init(b_xfull, NW);
     mbar_init(b_xfree, NW);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
 
-  // =========================================================================== producer warp
+  // =========================================================================== DMA warp (one lane)
+  // item n: (1) stage-input tile into y slot n % NY once its previous readers are done;
+  //         (2) outputs of item n - NUA (staged in place in slot n % NUA by the compute warps) -> global;
+  //         (3) u0 / acc of item n into that slot (or just "slot is free" when the stage loads neither).
   if (warp == NW) {
     if (lane == 0) {
+      auto store_item = [&](long long m) {   // outputs of item m
+        const int su = (int)(m % NUA);
+        const int iz0 = (int)((blockIdx.x + (m / nchunks) * gridDim.x) * TZ), c0 = (int)(m % nchunks) * VC;
+        mbar_wait_backoff(b_out_ready + 8 * su, (uint32_t)((m / NUA) & 1));
+        const uint32_t src = s_ua + su * NARR * SM::PTILE;
+        tma_store_3d(&tm_out, src, c0, iz0, 0);
+        if constexpr (KT::WRITE_ACC) tma_store_3d(&tm_acc, src + SM::PTILE, c0, iz0, 0);
+        tma_store_commit();
+        tma_store_wait_read();   // the slot may be overwritten from here on
+      };
       long long tile = blockIdx.x;
       int ch = 0;
       for (long long n = 0; n < nitems; ++n) {
@@ -264,16 +295,21 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
         mbar_wait_backoff(b_empty_y + 8 * sy, (uint32_t)(((n / NY) & 1) ^ 1));
         mbar_expect_tx(b_full_y + 8 * sy, SM::YTILE);
         tma_load_3d(s_y + sy * SM::YTILE, &tm_y, b_full_y + 8 * sy, ch * VC, iz0 + G - H, 0);
-        if constexpr (NARR > 0) {
-          const int su = (int)(n % NUA);
-          mbar_wait_backoff(b_empty_ua + 8 * su, (uint32_t)(((n / NUA) & 1) ^ 1));
-          mbar_expect_tx(b_full_ua + 8 * su, NARR * SM::PTILE);
-          uint32_t dst = s_ua + su * NARR * SM::PTILE;
-          if constexpr (KT::LOAD_U0) { tma_load_3d(dst, &tm_u0, b_full_ua + 8 * su, ch * VC, iz0 + G, 0); dst += SM::PTILE; }
-          if constexpr (KT::LOAD_ACC) tma_load_3d(dst, &tm_acc, b_full_ua + 8 * su, ch * VC, iz0 + G, 0);
+        if (n >= NUA) store_item(n - NUA);
+        const int su = (int)(n % NUA);
+        if constexpr (KT::NLOAD > 0) {
+          mbar_expect_tx(b_full_ua + 8 * su, KT::NLOAD * SM::PTILE);
+          const uint32_t dst = s_ua + su * NARR * SM::PTILE;
+          if constexpr (KT::LOAD_U0) tma_load_3d(dst, &tm_u0, b_full_ua + 8 * su, ch * VC, iz0, 0);
+          if constexpr (KT::LOAD_ACC)
+            tma_load_3d(dst + KT::ACC_LOAD_ARR * SM::PTILE, &tm_acc, b_full_ua + 8 * su, ch * VC, iz0, 0);
+        } else {
+          mbar_arrive(b_full_ua + 8 * su);   // nothing to load: the slot is free for staging
         }
         if (++ch == nchunks) { ch = 0; tile += gridDim.x; }
       }
+      for (long long m = nitems > NUA ? nitems - NUA : 0; m < nitems; ++m) store_item(m);
+      tma_store_wait_all();
     }
     return;
   }
@@ -281,13 +317,13 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
   // =========================================================================== compute warps
   const int row0 = warp * S;
   double macc = 0.0;      // running moment (one (row, quantity) per valid lane, see butterfly_reduce)
-  // lane l < 6S holds mu * moment (l % 6) of row row0 + l / 6 of the stage input; the next tile's values are
-  // fetched one tile ahead so that their latency is never exposed
+  // lane l < 6S holds moment (l % 6) of row row0 + l / 6 of the stage input; the next tile's values are
+  // fetched one tile ahead (and only touched at the next tile) so that their latency is never exposed
   auto load_min = [&](long long t) {
     double m = 0.0;
     if (lane < 6 * S && t < ntiles) {
       const long long iz = t * TZ + row0 + lane / 6;
-      if (iz < p.nz) m = p.mu * __ldg(p.mom_in + (long long)(lane % 6) * p.nz + iz);
+      if (iz < p.nz) m = __ldg(p.mom_in + (long long)(lane % 6) * p.nz + iz);
     }
     return m;
   };
@@ -297,20 +333,21 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
   for (long long n = 0; n < nitems; ++n) {
     const long long iz0 = tile * TZ;
     if (ch == 0) {
-      min_cur = min_next;
+      min_cur = p.mu * min_next;
       min_next = load_min(tile + gridDim.x);
     }
-    const int sy = (int)(n % NY);
-    const uint32_t Ty = s_y + sy * SM::YTILE + lane * 8;   // + ((c * ROWS + r) * 32) * 8
+    const int sy = (int)(n % NY), su = (int)(n % NUA);
+    const uint32_t Ty = s_y + sy * SM::YTILE + lane * 8;                  // + ((c * ROWS + r) * 32) * 8
+    const uint32_t Tu = s_ua + su * NARR * SM::PTILE + lane * 8;          // + ((c * TZ + r) * 32) * 8
+    const uint32_t Ta_in = Tu + KT::ACC_LOAD_ARR * SM::PTILE, Ta_out = Tu + SM::PTILE;
     const int j = ch * VC + lane;
     const bool active = j < p.nv;
     // v_j = -1 + (j + 1/2) dv, formed without contraction
     const double v = __dadd_rn(-1.0, __dmul_rn((double)j + 0.5, p.dv));
     mbar_wait(b_full_y + 8 * sy, (uint32_t)((n / NY) & 1));
 
-    // ---- S2 (WENO7): right-interface fluxes of my rows, exchanged with the neighbouring warps
+    // ---- S2 (WENO7): right-interface fluxes of my rows, published for the neighbouring warp
     double FR[SCHEME == 1 ? S : 1][8];
-    double FL[8];
     double nvz = 0.0, cadv_v = 0.0;
     if constexpr (SCHEME == 1) {
       nvz = v * p.ninv_dz;
@@ -351,30 +388,11 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
     // broadcast helper: mu * moment q of my row s
     auto mom = [&](int s, int q) { return __shfl_sync(0xffffffffu, min_cur, s * 6 + q); };
 
-    if constexpr (SCHEME == 1) {
-      mbar_wait(b_xfull, (uint32_t)(n & 1));
-      if (warp == 0) {
-#pragma unroll
-        for (int c = 0; c < 8; ++c) FL[c] = lds(s_xb + (c * VC + lane) * 8);
-      } else {
-#pragma unroll
-        for (int c = 0; c < 8; ++c) FL[c] = lds(s_x + (((warp - 1) * 8 + c) * VC + lane) * 8);
-      }
-      __syncwarp();
-      if (lane == 0) mbar_arrive(b_xfree);
-    }
-
-    uint32_t Tu = 0, Ta = 0;
-    if constexpr (NARR > 0) {
-      const int su = (int)(n % NUA);
-      Tu = s_ua + su * NARR * SM::PTILE + lane * 8;
-      Ta = Tu + (KT::LOAD_U0 ? SM::PTILE : 0u);
-      mbar_wait(b_full_ua + 8 * su, (uint32_t)((n / NUA) & 1));
-    }
-
     double mred[6 * S];
+    // rows in descending order: only row 0 needs the neighbour's flux, so its wait comes last
 #pragma unroll
-    for (int s = 0; s < S; ++s) {
+    for (int sd = 0; sd < S; ++sd) {
+      const int s = S - 1 - sd;
       const int row = row0 + s;
       const long long iz = iz0 + row;
       const bool act = active && (iz < p.nz);
@@ -382,19 +400,6 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
       double yc[8], k[8];
 #pragma unroll
       for (int c = 0; c < 8; ++c) yc[c] = lds(Ty + ((c * ROWS + tr) * VC) * 8);
-
-      // ---- S2: advection
-      if constexpr (SCHEME == 0) {
-#pragma unroll
-        for (int c = 0; c < 8; ++c) {
-          const uint32_t b = Ty + ((c * ROWS + tr) * VC) * 8;
-          k[c] = cosenu_math::fd4_ko3(lds(b - 2 * VC * 8), lds(b - VC * 8), yc[c], lds(b + VC * 8), lds(b + 2 * VC * 8),
-                                      cadv_v, p.cko);
-        }
-      } else {
-#pragma unroll
-        for (int c = 0; c < 8; ++c) k[c] = (FR[s][c] - (s == 0 ? FL[c] : FR[s > 0 ? s - 1 : 0][c])) * nvz;
-      }
 
       // ---- S3: Hamiltonian from the moments (mu folded in), commutator
       {
@@ -409,39 +414,67 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
           const int o = 4 * sp;
           const double dl = yc[o] - yc[o + 1];
           const double Tt = 2.0 * fma(Bi, yc[o + 2], -Br * yc[o + 3]);
-          k[o] += Tt;
-          k[o + 1] -= Tt;
-          k[o + 2] += fma(A, yc[o + 3], -Bi * dl);
-          k[o + 3] += fma(Br, dl, -A * yc[o + 2]);
+          k[o] = Tt;
+          k[o + 1] = -Tt;
+          k[o + 2] = fma(A, yc[o + 3], -Bi * dl);
+          k[o + 3] = fma(Br, dl, -A * yc[o + 2]);
         }
       }
 
-      // ---- S4: RK combine and stores
-      double out[8];
-      const long long gidx = (iz + G) * p.nvp + j;
-#pragma unroll
-      for (int c = 0; c < 8; ++c) {
-        double u0v = yc[c], accb;
-        if constexpr (KT::LOAD_U0) u0v = lds(Tu + ((c * TZ + row) * VC) * 8);
-        if constexpr (KIND == FIRST || KIND == FIRST_LEAN) accb = yc[c];
-        else if constexpr (KIND == MID_REBUILD) accb = fma(yc[c] - u0v, 1.0 / 3.0, u0v);  // u0 + (dt/6) k1
-        else accb = lds(Ta + ((c * TZ + row) * VC) * 8);
-        const double base = (KIND == LAST) ? accb : u0v;
-        out[c] = act ? fma(p.cy, k[c], base) : 0.0;
-        k[c] = fma(p.ca, k[c], accb);   // new accumulator value
-      }
-      if (act) {
+      // ---- S2: advection
+      if constexpr (SCHEME == 0) {
 #pragma unroll
         for (int c = 0; c < 8; ++c) {
-          double* yo = p.y_out + c * p.comp_stride + gidx;
-          *yo = out[c];
-          if constexpr (KT::WRITE_ACC) p.acc_out[c * p.comp_stride + gidx] = k[c];
+          const uint32_t b = Ty + ((c * ROWS + tr) * VC) * 8;
+          k[c] += cosenu_math::fd4_ko3(lds(b - 2 * VC * 8), lds(b - VC * 8), yc[c], lds(b + VC * 8), lds(b + 2 * VC * 8),
+                                       cadv_v, p.cko);
         }
-        if (iz < G) {                      // right ghost copy of the first rows
+      } else {
+        if (s == 0) {
+          double FL[8];
+          mbar_wait(b_xfull, (uint32_t)(n & 1));
+          if (warp == 0) {
+#pragma unroll
+            for (int c = 0; c < 8; ++c) FL[c] = lds(s_xb + (c * VC + lane) * 8);
+          } else {
+#pragma unroll
+            for (int c = 0; c < 8; ++c) FL[c] = lds(s_x + (((warp - 1) * 8 + c) * VC + lane) * 8);
+          }
+          __syncwarp();
+          if (lane == 0) mbar_arrive(b_xfree);
+#pragma unroll
+          for (int c = 0; c < 8; ++c) k[c] = fma(FR[0][c] - FL[c], nvz, k[c]);
+        } else {
+#pragma unroll
+          for (int c = 0; c < 8; ++c) k[c] = fma(FR[s][c] - FR[s > 0 ? s - 1 : 0][c], nvz, k[c]);
+        }
+      }
+
+      // ---- S4: RK combine; the outputs are staged in place in the u0/acc slot for the TMA store
+      if (sd == 0) mbar_wait(b_full_ua + 8 * su, (uint32_t)((n / NUA) & 1));
+      double out[8];
+#pragma unroll
+      for (int c = 0; c < 8; ++c) {
+        const uint32_t cell = ((c * TZ + row) * VC) * 8;
+        double u0v = yc[c], accb;
+        if constexpr (KT::LOAD_U0) u0v = lds(Tu + cell);
+        if constexpr (KIND == FIRST || KIND == FIRST_LEAN) accb = yc[c];
+        else if constexpr (KIND == MID_REBUILD) accb = fma(yc[c] - u0v, 1.0 / 3.0, u0v);  // u0 + (dt/6) k1
+        else accb = lds(Ta_in + cell);
+        const double base = (KIND == LAST) ? accb : u0v;
+        const double o = fma(p.cy, k[c], base);
+        sts(Tu + cell, o);
+        if constexpr (KT::WRITE_ACC) sts(Ta_out + cell, fma(p.ca, k[c], accb));
+        out[c] = act ? o : 0.0;
+      }
+      // periodic ghost rows of y_out (device rows outside 0..nz-1) are written directly
+      if (act && (iz < G || iz >= p.nz - G)) {
+        const long long gidx = (iz + G) * p.nvp + j;
+        if (iz < G) {
 #pragma unroll
           for (int c = 0; c < 8; ++c) p.y_out[c * p.comp_stride + gidx + p.nz * p.nvp] = out[c];
         }
-        if (iz >= p.nz - G) {              // left ghost copy of the last rows
+        if (iz >= p.nz - G) {
 #pragma unroll
           for (int c = 0; c < 8; ++c) p.y_out[c * p.comp_stride + gidx - p.nz * p.nvp] = out[c];
         }
@@ -456,11 +489,12 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
       mred[6 * s + 5] = v * mred[6 * s + 4];
     }
 
-    // all shared-memory reads of this item are done: hand the slots back to the producer
+    // all reads of the stage-input slot are done, and my outputs are staged: tell the DMA warp
+    fence_proxy_async();
     __syncwarp();
     if (lane == 0) {
       mbar_arrive(b_empty_y + 8 * sy);
-      if constexpr (NARR > 0) mbar_arrive(b_empty_ua + 8 * (int)(n % NUA));
+      mbar_arrive(b_out_ready + 8 * su);
     }
 
     int midx;
