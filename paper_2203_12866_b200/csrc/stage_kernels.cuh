@@ -65,7 +65,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "{\n"
       ".reg .pred p;\n"
       "WAIT_%=:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, 0x989680;\n"
       "@p bra DONE_%=;\n"
       "bra WAIT_%=;\n"
       "DONE_%=:\n"
@@ -139,10 +139,13 @@ struct StageSmem {
   static constexpr int NARR = KindTraits<KIND>::NARR;
   static constexpr uint32_t off_y = 0;
   static constexpr uint32_t off_ua = off_y + NY * YTILE;               // [NUA][NARR][PTILE]
-  static constexpr uint32_t off_x = off_ua + NUA * NARR * PTILE;       // [NSEG][8][32] exchange (WENO)
-  static constexpr uint32_t off_xb = off_x + (SCHEME == 1 ? NSEG * 8u * VC * 8u : 0u);  // [8][32] boundary (WENO)
-  static constexpr uint32_t off_bar = off_xb + (SCHEME == 1 ? 8u * VC * 8u : 0u);
-  static constexpr uint32_t nbar = 2 * NY + 2 * NUA + 2;
+  static constexpr int XBUF = NSEG <= 8 ? 2 : 1;                        // copies of the flux exchange buffers
+  static constexpr uint32_t XSZ = NSEG * 8u * VC * 8u, XBSZ = 8u * VC * 8u;
+  static constexpr uint32_t off_x = off_ua + NUA * NARR * PTILE;       // [XBUF][NSEG][8][32] exchange (WENO)
+  static constexpr uint32_t off_xb = off_x + (SCHEME == 1 ? XBUF * XSZ : 0u);  // [XBUF][8][32] boundary (WENO)
+  static constexpr uint32_t off_bar = off_xb + (SCHEME == 1 ? XBUF * XBSZ : 0u);
+  // full_y[NY] empty_y[NY] full_ua[NUA] out_ready[NUA] | xf[XBUF][NSEG] xr[XBUF][NSEG] xbf[XBUF] xbr[XBUF]
+  static constexpr uint32_t nbar = 2 * NY + 2 * NUA + XBUF * (2 * NSEG + 2);
   static constexpr size_t bytes = off_bar + 8 * nbar + 128;
 };
 
@@ -252,9 +255,13 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
   const uint32_t sbase = (smem_u32(smem_raw) + 127u) & ~127u;
   const uint32_t s_y = sbase + SM::off_y, s_ua = sbase + SM::off_ua, s_x = sbase + SM::off_x, s_xb = sbase + SM::off_xb;
   const uint32_t s_bar = sbase + SM::off_bar;
-  // barriers: full_y[NY], empty_y[NY], full_ua[NUA], out_ready[NUA], xfull, xfree
+  constexpr int XBUF = SM::XBUF;
+  // barriers: full_y[NY], empty_y[NY], full_ua[NUA], out_ready[NUA]; flux exchange between neighbouring
+  // warps is pairwise: xf[b][w] "warp w published its last flux", xr[b][w] "warp w+1 has read it",
+  // xbf[b] "the 8 boundary pieces are published", xbr[b] "warp 0 has read them"
   const uint32_t b_full_y = s_bar, b_empty_y = s_bar + 8 * NY, b_full_ua = s_bar + 16 * NY,
-                 b_out_ready = s_bar + 16 * NY + 8 * NUA, b_xfull = s_bar + 16 * NY + 16 * NUA, b_xfree = b_xfull + 8;
+                 b_out_ready = s_bar + 16 * NY + 8 * NUA, b_xf = s_bar + 16 * NY + 16 * NUA,
+                 b_xr = b_xf + 8 * XBUF * NSEG, b_xbf = b_xr + 8 * XBUF * NSEG, b_xbr = b_xbf + 8 * XBUF;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int nchunks = (p.nv + VC - 1) / VC;
@@ -265,8 +272,10 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
   if (threadIdx.x == 0) {
     for (int b = 0; b < NY; ++b) { mbar_init(b_full_y + 8 * b, 1); mbar_init(b_empty_y + 8 * b, NW); }
     for (int b = 0; b < NUA; ++b) { mbar_init(b_full_ua + 8 * b, 1); mbar_init(b_out_ready + 8 * b, NW); }
-    mbar_init(b_xfull, NW);
-    mbar_init(b_xfree, NW);
+    if constexpr (SCHEME == 1) {
+      for (int b = 0; b < XBUF * NSEG; ++b) { mbar_init(b_xf + 8 * b, 1); mbar_init(b_xr + 8 * b, 1); }
+      for (int b = 0; b < XBUF; ++b) { mbar_init(b_xbf + 8 * b, 8); mbar_init(b_xbr + 8 * b, 1); }
+    }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -355,13 +364,27 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
       const uint32_t Tw = Ty + row0 * (VC * 8);
       const uint32_t Tc = Ty + (warp & 7) * (ROWS * VC * 8);   // boundary piece: component `warp` (warps 0..7)
       const unsigned mpos = __ballot_sync(0xffffffffu, v >= 0.0);
-      double FB = 0.0;
+      const int xb = (int)(n % XBUF);                       // exchange buffer of this item
+      const uint32_t xpar = (uint32_t)((n / XBUF) & 1);     // phase parity of its barriers
+      // (a) my piece of the tile's left boundary flux first, so that warp 0 never waits for it
+      if (warp < 8) {
+        double FB;
+        if (mpos == 0xffffffffu) FB = weno_boundary<1, ROWS, H>(Tc, bm);
+        else if (mpos == 0u) FB = weno_boundary<-1, ROWS, H>(Tc, bm);
+        else {
+          const double bp = weno_boundary_slow<1, ROWS, H>(Tc, bm), bn = weno_boundary_slow<-1, ROWS, H>(Tc, bm);
+          FB = v >= 0.0 ? bp : bn;
+        }
+        mbar_wait(b_xbr + 8 * xb, xpar ^ 1);   // warp 0 has read the previous contents
+        sts(s_xb + xb * SM::XBSZ + (warp * VC + lane) * 8, FB);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(b_xbf + 8 * xb);
+      }
+      // (b) the right-interface fluxes of my rows
       if (mpos == 0xffffffffu) {
         weno_rows<1, S, ROWS, H>(Tw, bm, FR);
-        if (warp < 8) FB = weno_boundary<1, ROWS, H>(Tc, bm);
       } else if (mpos == 0u) {
         weno_rows<-1, S, ROWS, H>(Tw, bm, FR);
-        if (warp < 8) FB = weno_boundary<-1, ROWS, H>(Tc, bm);
       } else {
         double Fp[S * 8], Fm[S * 8];
         weno_rows_slow<1, S, ROWS, H>(Tw, bm, Fp);
@@ -370,17 +393,15 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
         for (int s = 0; s < S; ++s)
 #pragma unroll
           for (int c = 0; c < 8; ++c) FR[s][c] = v >= 0.0 ? Fp[s * 8 + c] : Fm[s * 8 + c];
-        if (warp < 8) {
-          const double bp = weno_boundary_slow<1, ROWS, H>(Tc, bm), bn = weno_boundary_slow<-1, ROWS, H>(Tc, bm);
-          FB = v >= 0.0 ? bp : bn;
-        }
       }
-      mbar_wait(b_xfree, (uint32_t)((n & 1) ^ 1));   // readers of the previous item are done
+      // (c) publish the flux of my last row for the warp that owns the next rows
+      if (warp < NW - 1) {
+        mbar_wait(b_xr + 8 * (xb * NSEG + warp), xpar ^ 1);   // it has read the previous contents
 #pragma unroll
-      for (int c = 0; c < 8; ++c) sts(s_x + ((warp * 8 + c) * VC + lane) * 8, FR[S - 1][c]);
-      if (warp < 8) sts(s_xb + (warp * VC + lane) * 8, FB);
-      __syncwarp();
-      if (lane == 0) mbar_arrive(b_xfull);
+        for (int c = 0; c < 8; ++c) sts(s_x + xb * SM::XSZ + ((warp * 8 + c) * VC + lane) * 8, FR[S - 1][c]);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(b_xf + 8 * (xb * NSEG + warp));
+      }
     } else {
       cadv_v = v * p.cadv;
     }
@@ -432,16 +453,21 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
       } else {
         if (s == 0) {
           double FL[8];
-          mbar_wait(b_xfull, (uint32_t)(n & 1));
+          const int xb = (int)(n % XBUF);
+          const uint32_t xpar = (uint32_t)((n / XBUF) & 1);
           if (warp == 0) {
+            mbar_wait(b_xbf + 8 * xb, xpar);
 #pragma unroll
-            for (int c = 0; c < 8; ++c) FL[c] = lds(s_xb + (c * VC + lane) * 8);
+            for (int c = 0; c < 8; ++c) FL[c] = lds(s_xb + xb * SM::XBSZ + (c * VC + lane) * 8);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(b_xbr + 8 * xb);
           } else {
+            mbar_wait(b_xf + 8 * (xb * NSEG + warp - 1), xpar);
 #pragma unroll
-            for (int c = 0; c < 8; ++c) FL[c] = lds(s_x + (((warp - 1) * 8 + c) * VC + lane) * 8);
+            for (int c = 0; c < 8; ++c) FL[c] = lds(s_x + xb * SM::XSZ + (((warp - 1) * 8 + c) * VC + lane) * 8);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(b_xr + 8 * (xb * NSEG + warp - 1));
           }
-          __syncwarp();
-          if (lane == 0) mbar_arrive(b_xfree);
 #pragma unroll
           for (int c = 0; c < 8; ++c) k[c] = fma(FR[0][c] - FL[c], nvz, k[c]);
         } else {
