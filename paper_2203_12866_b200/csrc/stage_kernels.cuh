@@ -73,23 +73,8 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "r"(parity)
       : "memory");
 }
-// the producer's wait: back off between probes so that the spin does not take issue slots from the compute warps
-__device__ __forceinline__ void mbar_wait_backoff(uint32_t bar, uint32_t parity) {
-  uint32_t done = 0;
-  while (true) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-        "selp.u32 %0, 1, 0, p;\n"
-        "}\n"
-        : "=r"(done)
-        : "r"(bar), "r"(parity)
-        : "memory");
-    if (done) break;
-    __nanosleep(128);
-  }
-}
+// the DMA warp's wait: same, kept separate so that the profile shows which side waits
+__device__ __forceinline__ void mbar_wait_backoff(uint32_t bar, uint32_t parity) { mbar_wait(bar, parity); }
 // 3-D tiled TMA load global -> shared, completion on an mbarrier
 __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1, int c2) {
   asm volatile(
@@ -325,7 +310,9 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
 
   // =========================================================================== compute warps
   const int row0 = warp * S;
-  double macc = 0.0;      // running moment (one (row, quantity) per valid lane, see butterfly_reduce)
+  double msum[6 * S];     // per-lane partial moments of the tile's output, summed over the chunks in order
+#pragma unroll
+  for (int q = 0; q < 6 * S; ++q) msum[q] = 0.0;
   // lane l < 6S holds moment (l % 6) of row row0 + l / 6 of the stage input; the next tile's values are
   // fetched one tile ahead (and only touched at the next tile) so that their latency is never exposed
   auto load_min = [&](long long t) {
@@ -409,7 +396,6 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
     // broadcast helper: mu * moment q of my row s
     auto mom = [&](int s, int q) { return __shfl_sync(0xffffffffu, min_cur, s * 6 + q); };
 
-    double mred[6 * S];
     // rows in descending order: only row 0 needs the neighbour's flux, so its wait comes last
 #pragma unroll
     for (int sd = 0; sd < S; ++sd) {
@@ -507,12 +493,15 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
       }
 
       // ---- S5: velocity moments of the produced state, D = rho - rhobar^*
-      mred[6 * s + 0] = (out[0] - out[1]) - (out[4] - out[5]);
-      mred[6 * s + 2] = out[2] - out[6];
-      mred[6 * s + 4] = out[3] + out[7];
-      mred[6 * s + 1] = v * mred[6 * s + 0];
-      mred[6 * s + 3] = v * mred[6 * s + 2];
-      mred[6 * s + 5] = v * mred[6 * s + 4];
+      {
+        const double dd = (out[0] - out[1]) - (out[4] - out[5]), dr = out[2] - out[6], di = out[3] + out[7];
+        msum[6 * s + 0] += dd;
+        msum[6 * s + 1] = fma(v, dd, msum[6 * s + 1]);
+        msum[6 * s + 2] += dr;
+        msum[6 * s + 3] = fma(v, dr, msum[6 * s + 3]);
+        msum[6 * s + 4] += di;
+        msum[6 * s + 5] = fma(v, di, msum[6 * s + 5]);
+      }
     }
 
     // all reads of the stage-input slot are done, and my outputs are staged: tell the DMA warp
@@ -523,16 +512,17 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
       mbar_arrive(b_out_ready + 8 * su);
     }
 
-    int midx;
-    bool mvalid;
-    butterfly_reduce<6 * S>(mred, lane, midx, mvalid);
-    macc += mred[0];
     if (++ch == nchunks) {
+      // end of the tile: reduce the partial moments over the lanes (fixed tree) and write them out
+      int midx;
+      bool mvalid;
+      butterfly_reduce<6 * S>(msum, lane, midx, mvalid);
       if (mvalid) {
         const long long iz = iz0 + row0 + midx / 6;
-        if (iz < p.nz) p.mom_out[(long long)(midx % 6) * p.nz + iz] = macc * p.dv;
+        if (iz < p.nz) p.mom_out[(long long)(midx % 6) * p.nz + iz] = msum[0] * p.dv;
       }
-      macc = 0.0;
+#pragma unroll
+      for (int q = 0; q < 6 * S; ++q) msum[q] = 0.0;
       ch = 0;
       tile += gridDim.x;
     }

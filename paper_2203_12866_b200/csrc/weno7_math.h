@@ -78,9 +78,11 @@ COSENU_HD Weno7Beam weno7_beam(double v, double eps) {
 }
 
 // the part of Algorithm 1 after the undivided differences: D[0..5], E[0..4], T[0..3] of the 7 cells
-// w[0..6] (D_k = w[k+1]-w[k], E_k = D[k+1]-D[k], T_k = E[k+1]-E[k]); ui = w[3].
+// w[0..6] (D_k = w[k+1]-w[k], E_k = D[k+1]-D[k], T_k = E[k+1]-E[k]); ui = w[3]; TTk = T_k^2 (shared
+// between neighbouring interfaces by weno7_face2).
 COSENU_HD double weno7_core(double ui, double D0, double D1, double D2, double D3, double E0, double E1, double E2,
-                            double E3, double E4, double T0, double T1, double T2, double T3, const Weno7Beam& bm) {
+                            double E3, double E4, double T0, double T3, double TT0, double TT1, double TT2, double TT3,
+                            const Weno7Beam& bm) {
   // A_r, s_r per sub-stencil: (x, p, q, t) = (D[3-r], E[3-r], E[4-r], T[3-r])
   const double A0 = fma(1.0 / 3.0, E4, fma(-5.0 / 6.0, E3, D3));
   const double A1 = fma(-1.0 / 6.0, E3, fma(2.0 / 3.0, E2, D2));
@@ -91,17 +93,18 @@ COSENU_HD double weno7_core(double ui, double D0, double D1, double D2, double D
   // qs_r = (240 A^2 + 260 s^2 + (781/3) t^2 + eps/v^2) / sqrt(d_r)
   constexpr double k0 = 2.9580398915498080213, k1 = 1.3944333775567926, k2 = 1.7078251276599330,
                    k3 = 5.9160797830996160426;
-  const double q0 = fma(240.0 * k0, A0 * A0, fma(260.0 * k0, s0 * s0, fma((781.0 / 3.0) * k0, T3 * T3, bm.e0)));
-  const double q1 = fma(240.0 * k1, A1 * A1, fma(260.0 * k1, ss12, fma((781.0 / 3.0) * k1, T2 * T2, bm.e1)));
-  const double q2 = fma(240.0 * k2, A2 * A2, fma(260.0 * k2, ss12, fma((781.0 / 3.0) * k2, T1 * T1, bm.e2)));
-  const double q3 = fma(240.0 * k3, A3 * A3, fma(260.0 * k3, s3 * s3, fma((781.0 / 3.0) * k3, T0 * T0, bm.e3)));
+  const double q0 = fma(240.0 * k0, A0 * A0, fma(260.0 * k0, s0 * s0, fma((781.0 / 3.0) * k0, TT3, bm.e0)));
+  const double q1 = fma(240.0 * k1, A1 * A1, fma(260.0 * k1, ss12, fma((781.0 / 3.0) * k1, TT2, bm.e1)));
+  const double q2 = fma(240.0 * k2, A2 * A2, fma(260.0 * k2, ss12, fma((781.0 / 3.0) * k2, TT1, bm.e2)));
+  const double q3 = fma(240.0 * k3, A3 * A3, fma(260.0 * k3, s3 * s3, fma((781.0 / 3.0) * k3, TT0, bm.e3)));
   const double Q0 = q0 * q0, Q1 = q1 * q1, Q2 = q2 * q2, Q3 = q3 * q3;
   const double Q01 = Q0 * Q1, Q23 = Q2 * Q3;
-  const double P0 = Q1 * Q23, P1 = Q0 * Q23, P2 = Q01 * Q3, P3 = Q01 * Q2;
-  const double den = (P0 + P1) + (P2 + P3);
+  // P_0 = Q1 Q23, P_1 = Q0 Q23, P_2 = Q01 Q3, P_3 = Q01 Q2, grouped:
+  //   den = Q23 (Q0 + Q1) + Q01 (Q2 + Q3),  num = Q23 (Q1 c0 + Q0 c1) + Q01 (Q3 c2 + Q2 c3)
   const double c0 = fma(1.0 / 6.0, s0, A0), c1 = fma(1.0 / 6.0, E2, A1), c2 = fma(1.0 / 6.0, E2, A2),
                c3 = fma(1.0 / 6.0, s3, A3);
-  const double num = fma(P0, c0, fma(P1, c1, fma(P2, c2, P3 * c3)));
+  const double den = fma(Q01, Q2 + Q3, Q23 * (Q0 + Q1));
+  const double num = fma(Q01, fma(Q3, c2, Q2 * c3), Q23 * fma(Q1, c0, Q0 * c1));
   return fma(num, 0.5 * fast_rcp2(den), ui);
 }
 
@@ -112,7 +115,7 @@ COSENU_HD double weno7_face(const double w[7], const Weno7Beam& bm) {
                D5 = w[6] - w[5];
   const double E0 = D1 - D0, E1 = D2 - D1, E2 = D3 - D2, E3 = D4 - D3, E4 = D5 - D4;
   const double T0 = E1 - E0, T1 = E2 - E1, T2 = E3 - E2, T3 = E4 - E3;
-  return weno7_core(w[3], D0, D1, D2, D3, E0, E1, E2, E3, E4, T0, T1, T2, T3, bm);
+  return weno7_core(w[3], D0, D1, D2, D3, E0, E1, E2, E3, E4, T0, T3, T0 * T0, T1 * T1, T2 * T2, T3 * T3, bm);
 }
 
 // two adjacent interfaces from 8 cells w[0..7] with shared differences:
@@ -122,8 +125,9 @@ COSENU_HD void weno7_face2(const double w[8], const Weno7Beam& bm, double& Fa, d
                D5 = w[6] - w[5], D6 = w[7] - w[6];
   const double E0 = D1 - D0, E1 = D2 - D1, E2 = D3 - D2, E3 = D4 - D3, E4 = D5 - D4, E5 = D6 - D5;
   const double T0 = E1 - E0, T1 = E2 - E1, T2 = E3 - E2, T3 = E4 - E3, T4 = E5 - E4;
-  Fa = weno7_core(w[3], D0, D1, D2, D3, E0, E1, E2, E3, E4, T0, T1, T2, T3, bm);
-  Fb = weno7_core(w[4], D1, D2, D3, D4, E1, E2, E3, E4, E5, T1, T2, T3, T4, bm);
+  const double TT0 = T0 * T0, TT1 = T1 * T1, TT2 = T2 * T2, TT3 = T3 * T3, TT4 = T4 * T4;
+  Fa = weno7_core(w[3], D0, D1, D2, D3, E0, E1, E2, E3, E4, T0, T3, TT0, TT1, TT2, TT3, bm);
+  Fb = weno7_core(w[4], D1, D2, D3, D4, E1, E2, E3, E4, E5, T1, T4, TT1, TT2, TT3, TT4, bm);
 }
 
 // FD4 + KO3 in difference form (Eq. (5)): returns
