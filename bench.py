@@ -32,8 +32,10 @@ METRIC = "(z,v) cell-updates/sec per RK4 step (fp64)"
 UNIT = "cell-updates/s"
 # algorithmic HBM bytes per cell per stage launch:
 # read stage input + u0 + acc, write stage output + acc, 64 B each
-BYTES_PER_CELL_STAGE = {"first": 192, "mid": 320, "last": 192}
-BYTES_PER_CELL_STEP = 1024
+# per RK formulation (cosenu.h COSENU_OPT_RK_FORM): bytes per cell of stages 1..4
+STAGE_BYTES = {0: [192, 320, 320, 192], 1: [128, 256, 320, 192], 2: [128, 192, 192, 320]}
+STAGE_KERNEL = {0: ["FIRST", "MID", "MID", "LAST"], 1: ["FIRST_LEAN", "MID_REBUILD", "MID", "LAST"],
+                2: ["FIRST_LEAN", "MID_NOACC", "MID_NOACC", "LAST_COMB"]}
 # dram__bytes_read.sum + dram__bytes_write.sum per MID-stage launch from the committed ncu capture
 # (profiles/), per workload; None until captured
 NCU_TRAFFIC_BYTES = {}
@@ -175,7 +177,7 @@ def run_ours(args):
     hnp = host.numpy()
     hnp[...] = inputs.fast_conversion_state(nz, nv, c["seed"] + rank) if c["kind"] == "fast" else \
         inputs.vacuum_check_state(nz, nv, c["seed"] + rank)
-    sim = B.Cosenu(nz, nv, c["L"], c["dt"], c["omega"], c["theta"], c["mu"], c["scheme"], lean_acc=bool(args.lean_acc),
+    sim = B.Cosenu(nz, nv, c["L"], c["dt"], c["omega"], c["theta"], c["mu"], c["scheme"], rk_form=args.rk_form,
                    variant=args.variant)
     sim.set_state(host)
     d0 = sim.diagnostics()
@@ -241,24 +243,25 @@ def run_ours(args):
         if world > 1:
             dist.destroy_process_group()
         return
-    # ---- roofline of the dominant kernel: the MID stage launch (stages 2 and 3: 320 B/cell algorithmic)
+    # ---- roofline of the dominant kernel = the stage launch with the longest average duration
     peak, peak_src = measured_peaks()
-    mid_ms = (stage_ms[1] + stage_ms[2]) / (2.0 * max(nst, 1))
-    kinds = ["first", "mid", "mid", "last"]
-    per_stage = [{"stage": k + 1, "avg_ms": stage_ms[k] / max(nst, 1),
-                  "GBps": BYTES_PER_CELL_STAGE[kinds[k]] * cells / (stage_ms[k] / max(nst, 1) * 1e-3) / 1e9}
-                 for k in range(4)] if nst else []
-    mid_bytes = (256 if args.lean_acc else 320)
-    achieved = mid_bytes * cells / (mid_ms * 1e-3) / 1e9 if nst else None
+    sb = STAGE_BYTES[args.rk_form]
+    step_bytes = sum(sb)
+    avg = [stage_ms[k] / max(nst, 1) for k in range(4)]
+    per_stage = [{"stage": k + 1, "kernel": STAGE_KERNEL[args.rk_form][k], "bytes_per_cell": sb[k], "avg_ms": avg[k],
+                  "GBps": sb[k] * cells / (avg[k] * 1e-3) / 1e9} for k in range(4)] if nst else []
+    dom = max(range(4), key=lambda k: avg[k]) if nst else 0
+    achieved = per_stage[dom]["GBps"] if nst else None
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak if achieved else None,
-                "traffic": NCU_TRAFFIC_BYTES.get(c["name"]), "peak_source": peak_src,
-                "kernel": "stage_kernel<%s, MID> (RK stages 2 and 3)" % ("WENO7" if c["scheme"] else "FD4_KO3"),
-                "algorithmic_bytes_per_launch": mid_bytes * cells, "avg_launch_ms": mid_ms,
-                "stage_kernel_share_of_step": sum(stage_ms) / max(nst, 1) / (ms / args.steps) if nst else None,
-                "per_stage": per_stage,
-                "step_model_GBps": (896 if args.lean_acc else BYTES_PER_CELL_STEP) * value / world / 1e9,
-                "step_model_frac": (896 if args.lean_acc else BYTES_PER_CELL_STEP) * value / world / 1e9 / peak}
+                "traffic": NCU_TRAFFIC_BYTES.get((c["name"], args.rk_form)), "peak_source": peak_src,
+                "kernel": "stage_kernel<%s, %s> (RK stage %d)" % ("WENO7" if c["scheme"] else "FD4_KO3",
+                                                                  STAGE_KERNEL[args.rk_form][dom], dom + 1),
+                "algorithmic_bytes_per_launch": sb[dom] * cells, "avg_launch_ms": avg[dom],
+                "stage_kernel_share_of_step": sum(avg) / (ms / args.steps) if nst else None,
+                "per_stage": per_stage, "bytes_per_cell_step": step_bytes,
+                "step_model_GBps": step_bytes * value / world / 1e9,
+                "step_model_frac": step_bytes * value / world / 1e9 / peak}
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         cpu, _, _, _ = oracle_sample(c)
@@ -268,7 +271,7 @@ def run_ours(args):
            "config": {"workload": c["name"], "scheme": "FV_WENO7" if c["scheme"] else "FD4_KO3", "nz": nz, "nv": nv,
                       "dt": c["dt"], "omega": c["omega"], "theta": c["theta"], "mu": c["mu"],
                       "state_bytes_per_copy": state_bytes, "l2": "inputs larger than L2 (no flush needed)",
-                      "parallelism": "replicas x%d" % world, "lean_acc": bool(args.lean_acc), "variant": args.variant},
+                      "parallelism": "replicas x%d" % world, "rk_form": args.rk_form, "variant": args.variant},
            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
            "checks": checks}
     print(json.dumps(out))
@@ -284,7 +287,7 @@ def main():
     ap.add_argument("--workload", default="cfg4", choices=["cfg0", "cfg1", "cfg2", "cfg3", "cfg4"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
-    ap.add_argument("--lean-acc", type=int, default=0)
+    ap.add_argument("--rk-form", type=int, default=2, choices=[0, 1, 2])
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

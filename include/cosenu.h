@@ -52,9 +52,12 @@ enum {
   COSENU_OPT_EPS_KO = 0,   /* Kreiss-Oliger strength eps_KO of Eq. (5); default 0.1; >= 0 */
   COSENU_OPT_WENO_EPS = 1, /* epsilon of Eq. (14); default 1e-6; 0 < eps <= 1e30 */
   COSENU_OPT_ADVECT = 2,   /* 0 switches the advection term off (commutator-only runs); default 1 */
-  COSENU_OPT_LEAN_ACC = 3, /* 1: stage 1 does not store the RK accumulator, stage 2 rebuilds k1 from
-                              (y2 - u0) 2/dt  (896 instead of 1024 B of traffic per cell-step, costs
-                              <= 1 ulp of the state per step); default 0 */
+  COSENU_OPT_RK_FORM = 3,  /* how the classical RK4 combination is carried between the 4 stage launches
+                              (same method, same result up to rounding; differs in HBM traffic per cell-step):
+                              0: accumulator array  ACC = u + dt/6 (k1 + 2k2 + 2k3), updated by every stage  (1024 B)
+                              1: as 0, but stage 1 does not store ACC; stage 2 rebuilds k1 from (y2 - u) 2/dt  (896 B)
+                              2: no accumulator: u+ = (y2 + 2 y3 + y4 - u)/3 + dt/6 k4 from the stage states   (832 B)
+                              default 2 */
   COSENU_OPT_STAGE_TIMING = 4, /* 1: bracket every stage launch with CUDA events on the handle's stream
                               (read with cosenu_stage_times); default 0 */
   COSENU_OPT_VARIANT = 5   /* kernel shape: 0 = 16 compute warps x 1 row (default), 1 = 8 compute warps x 2 rows;

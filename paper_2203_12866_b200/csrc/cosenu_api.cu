@@ -38,7 +38,7 @@ struct cosenu {
   int64_t nz; int32_t nv; int nvp;
   double L, dt, omega, theta, mu; int scheme;
   double eps_ko = 0.1, weno_eps = 1e-6;
-  int advect = 1, lean_acc = 0, stage_timing = 0;
+  int advect = 1, rk_form = 2, stage_timing = 0;   // rk_form: 0 accumulator, 1 lean accumulator, 2 accumulator-free
   double dz, dv;
   int device = 0;
   int variant = 0;       // kernel shape variant (COSENU_OPT_VARIANT)
@@ -52,7 +52,7 @@ struct cosenu {
   double *d_pref = nullptr, *d_p0ref = nullptr, *d_refpart = nullptr, *d_diagpart = nullptr;
   int64_t comp_stride = 0; size_t state_elems = 0;
   int mcur = 0;  // M[mcur] holds the moments of U
-  CUtensorMap tm_U, tm_Y1, tm_Y2;   // stage-input boxes [8][TZ+2H][32]
+  CUtensorMap tm_U, tm_Y1, tm_Y2, tm_ACC;   // stage-input boxes [8][TZ+2H][32]
   CUtensorMap tp_U, tp_Y1, tp_Y2, tp_ACC;   // rows 0..nz-1 only, boxes [8][TZ][32]: u0 / acc loads, output stores
   bool maps_ready = false;
 
@@ -145,6 +145,7 @@ int ensure_workspace(cosenu* h) {
   if ((rc = make_map(h, enc, &h->tm_U, h->U, rows, true))) return rc;
   if ((rc = make_map(h, enc, &h->tm_Y1, h->Y1, rows, true))) return rc;
   if ((rc = make_map(h, enc, &h->tm_Y2, h->Y2, rows, true))) return rc;
+  if ((rc = make_map(h, enc, &h->tm_ACC, h->ACC, rows, true))) return rc;
   if ((rc = make_map(h, enc, &h->tp_U, h->U, TZ_ALL, false))) return rc;
   if ((rc = make_map(h, enc, &h->tp_Y1, h->Y1, TZ_ALL, false))) return rc;
   if ((rc = make_map(h, enc, &h->tp_Y2, h->Y2, TZ_ALL, false))) return rc;
@@ -154,7 +155,8 @@ int ensure_workspace(cosenu* h) {
 }
 
 template <int SCHEME, int KIND, int TZ, int NSEG, int NY, int NUA>
-int launch_one(cosenu* h, const CUtensorMap& map, const CUtensorMap& omap, const StageParams& p) {
+int launch_one(cosenu* h, const CUtensorMap& map, const CUtensorMap& omap, const CUtensorMap& a1, const CUtensorMap& a2,
+               const StageParams& p) {
   auto kern = stage_kernel<SCHEME, KIND, TZ, NSEG, NY, NUA>;
   constexpr size_t smem = StageSmem<SCHEME, KIND, TZ, NSEG, NY, NUA>::bytes;
   static_assert(smem <= 232448, "over the 227 KB shared-memory limit of a CTA");
@@ -165,30 +167,34 @@ int launch_one(cosenu* h, const CUtensorMap& map, const CUtensorMap& omap, const
   }
   const long long ntiles = (h->nz + TZ - 1) / TZ;
   const unsigned grid = (unsigned)(ntiles < h->num_sms ? ntiles : h->num_sms);   // persistent: one CTA per SM
-  kern<<<grid, NSEG * 32 + 32, smem, h->stream>>>(map, h->tp_U, h->tp_ACC, omap, p);
+  kern<<<grid, NSEG * 32 + 32, smem, h->stream>>>(map, h->tp_U, a1, a2, omap, p);
   CK(cudaGetLastError());
   h->launches++;
   return COSENU_OK;
 }
 
 template <int SCHEME, int TZ, int NSEG, int NY, int NUA>
-int launch_kind(cosenu* h, int kind, const CUtensorMap& map, const CUtensorMap& omap, const StageParams& p) {
+int launch_kind(cosenu* h, int kind, const CUtensorMap& map, const CUtensorMap& omap, const CUtensorMap& a1,
+                const CUtensorMap& a2, const StageParams& p) {
   switch (kind) {
-    case FIRST: return launch_one<SCHEME, FIRST, TZ, NSEG, NY, NUA>(h, map, omap, p);
-    case FIRST_LEAN: return launch_one<SCHEME, FIRST_LEAN, TZ, NSEG, NY, NUA>(h, map, omap, p);
-    case MID: return launch_one<SCHEME, MID, TZ, NSEG, NY, NUA>(h, map, omap, p);
-    case MID_REBUILD: return launch_one<SCHEME, MID_REBUILD, TZ, NSEG, NY, NUA>(h, map, omap, p);
-    default: return launch_one<SCHEME, LAST, TZ, NSEG, NY, NUA>(h, map, omap, p);
+    case FIRST: return launch_one<SCHEME, FIRST, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
+    case FIRST_LEAN: return launch_one<SCHEME, FIRST_LEAN, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
+    case MID: return launch_one<SCHEME, MID, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
+    case MID_REBUILD: return launch_one<SCHEME, MID_REBUILD, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
+    case LAST: return launch_one<SCHEME, LAST, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
+    case MID_NOACC: return launch_one<SCHEME, MID_NOACC, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
+    default: return launch_one<SCHEME, LAST_COMB, TZ, NSEG, NY, 1>(h, map, omap, a1, a2, p);   // 3 staged arrays: one slot
   }
 }
 
-int launch_stage(cosenu* h, int kind, const CUtensorMap& map, const CUtensorMap& omap, const StageParams& p) {
+int launch_stage(cosenu* h, int kind, const CUtensorMap& map, const CUtensorMap& omap, const CUtensorMap& a1,
+                 const CUtensorMap& a2, const StageParams& p) {
   if (h->scheme == COSENU_FD4_KO3) {
-    if (h->variant == 1) return launch_kind<0, TZ_ALL, 8, 2, 2>(h, kind, map, omap, p);
-    return launch_kind<0, TZ_ALL, 16, 2, 2>(h, kind, map, omap, p);
+    if (h->variant == 1) return launch_kind<0, TZ_ALL, 8, 2, 2>(h, kind, map, omap, a1, a2, p);
+    return launch_kind<0, TZ_ALL, 16, 2, 2>(h, kind, map, omap, a1, a2, p);
   }
-  if (h->variant == 1) return launch_kind<1, TZ_ALL, 8, 2, 1>(h, kind, map, omap, p);
-  return launch_kind<1, TZ_ALL, 16, 2, 1>(h, kind, map, omap, p);
+  if (h->variant == 1) return launch_kind<1, TZ_ALL, 8, 2, 1>(h, kind, map, omap, a1, a2, p);
+  return launch_kind<1, TZ_ALL, 16, 2, 1>(h, kind, map, omap, a1, a2, p);
 }
 
 StageParams base_params(const cosenu* h) {
@@ -245,25 +251,32 @@ int one_step(cosenu* h) {
   }
   double* Min = h->M[h->mcur];
   double* Mout = h->M[h->mcur ^ 1];
-  // stage 1: k1 = RHS(U); Y1 = U + dt/2 k1; ACC = U + dt/6 k1
+  const int form = h->rk_form;
+  // buffers: U -> Y1 -> Y2 -> (Y1 | ACC) -> U.  In the accumulator-free form the fourth state buffer (ACC)
+  // holds Y4, so that Y2 (in Y1) and Y3 (in Y2) are still there for the final combination.
+  // stage 1: k1 = RHS(U); Y1 = U + dt/2 k1; [ACC = U + dt/6 k1]
   p.y_out = h->Y1; p.acc_out = h->ACC; p.mom_in = Min; p.mom_out = Mout;
   p.cy = 0.5 * dt; p.ca = dt / 6.0;
-  if ((rc = launch_stage(h, h->lean_acc ? FIRST_LEAN : FIRST, h->tm_U, h->tp_Y1, p))) return rc;
+  if ((rc = launch_stage(h, form == 0 ? FIRST : FIRST_LEAN, h->tm_U, h->tp_Y1, h->tp_ACC, h->tp_ACC, p))) return rc;
   if (tm) CK(cudaEventRecord(ev[1], h->stream));
-  // stage 2: k2 = RHS(Y1); Y2 = U + dt/2 k2; ACC += dt/3 k2
+  // stage 2: k2 = RHS(Y1); Y2 = U + dt/2 k2; [ACC += dt/3 k2]
   p.y_out = h->Y2; p.acc_out = h->ACC; p.mom_in = Mout; p.mom_out = Min;
   p.cy = 0.5 * dt; p.ca = dt / 3.0;
-  if ((rc = launch_stage(h, h->lean_acc ? MID_REBUILD : MID, h->tm_Y1, h->tp_Y2, p))) return rc;
+  if ((rc = launch_stage(h, form == 0 ? MID : (form == 1 ? MID_REBUILD : MID_NOACC), h->tm_Y1, h->tp_Y2, h->tp_ACC,
+                         h->tp_ACC, p))) return rc;
   if (tm) CK(cudaEventRecord(ev[2], h->stream));
-  // stage 3: k3 = RHS(Y2); Y1 = U + dt k3; ACC += dt/3 k3
-  p.y_out = h->Y1; p.mom_in = Min; p.mom_out = Mout;
+  // stage 3: k3 = RHS(Y2); Y4 = U + dt k3 (into Y1, or into ACC in the accumulator-free form); [ACC += dt/3 k3]
+  p.y_out = form == 2 ? h->ACC : h->Y1; p.mom_in = Min; p.mom_out = Mout;
   p.cy = dt; p.ca = dt / 3.0;
-  if ((rc = launch_stage(h, MID, h->tm_Y2, h->tp_Y1, p))) return rc;
+  if ((rc = launch_stage(h, form == 2 ? MID_NOACC : MID, h->tm_Y2, form == 2 ? h->tp_ACC : h->tp_Y1, h->tp_ACC,
+                         h->tp_ACC, p))) return rc;
   if (tm) CK(cudaEventRecord(ev[3], h->stream));
-  // stage 4: k4 = RHS(Y1); U = ACC + dt/6 k4
+  // stage 4: k4 = RHS(Y4); U = ACC + dt/6 k4   or   U = (Y2 + 2 Y3 + Y4 - U)/3 + dt/6 k4
   p.y_out = h->U; p.acc_out = nullptr; p.mom_in = Mout; p.mom_out = Min;
   p.cy = dt / 6.0; p.ca = 0.0;
-  if ((rc = launch_stage(h, LAST, h->tm_Y1, h->tp_U, p))) return rc;
+  if (form == 2) rc = launch_stage(h, LAST_COMB, h->tm_ACC, h->tp_U, h->tp_Y1, h->tp_Y2, p);
+  else rc = launch_stage(h, LAST, h->tm_Y1, h->tp_U, h->tp_ACC, h->tp_ACC, p);
+  if (rc) return rc;
   if (tm) CK(cudaEventRecord(ev[4], h->stream));
   // moments of the new U are in Min = M[mcur] again
   h->t += dt; h->step += 1;
@@ -388,7 +401,7 @@ extern "C" int cosenu_set_option(cosenu_t* h, int key, double value) {
     case COSENU_OPT_EPS_KO: if (!(value >= 0) || !std::isfinite(value)) break; h->eps_ko = value; return COSENU_OK;
     case COSENU_OPT_WENO_EPS: if (!(value > 0) || !(value <= 1e30)) break; h->weno_eps = value; return COSENU_OK;
     case COSENU_OPT_ADVECT: h->advect = value != 0; return COSENU_OK;
-    case COSENU_OPT_LEAN_ACC: h->lean_acc = value != 0; return COSENU_OK;
+    case COSENU_OPT_RK_FORM: if (value != 0 && value != 1 && value != 2) break; h->rk_form = (int)value; return COSENU_OK;
     case COSENU_OPT_VARIANT: if (value != 0 && value != 1) break; h->variant = (int)value; return COSENU_OK;
     case COSENU_OPT_STAGE_TIMING: {
       int rc = drain_events(h);

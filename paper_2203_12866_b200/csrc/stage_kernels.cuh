@@ -32,7 +32,12 @@ namespace cosenu_dev {
 constexpr int G = 4;    // ghost rows per side in the device layout
 constexpr int VC = 32;  // beams per chunk = lanes of a warp
 
-enum StageKind { FIRST = 0, FIRST_LEAN = 1, MID = 2, MID_REBUILD = 3, LAST = 4 };
+// RK4 formulations:
+//  accumulator form  : FIRST, MID, MID, LAST                    1024 B per cell-step
+//  lean accumulator  : FIRST_LEAN, MID_REBUILD, MID, LAST        896 B
+//  accumulator-free  : FIRST_LEAN, MID_NOACC, MID_NOACC, LAST_COMB   832 B:
+//      Y2 = U + dt/2 k1, Y3 = U + dt/2 k2, Y4 = U + dt k3,  U+ = (Y2 + 2 Y3 + Y4 - U)/3 + dt/6 k4
+enum StageKind { FIRST = 0, FIRST_LEAN = 1, MID = 2, MID_REBUILD = 3, LAST = 4, MID_NOACC = 5, LAST_COMB = 6 };
 
 struct StageParams {
   double* y_out;          // next stage input (FIRST/MID) or the new U (LAST)
@@ -104,13 +109,14 @@ __device__ __forceinline__ void sts(uint32_t addr, double v) {
 
 template <int KIND>
 struct KindTraits {
-  static constexpr bool LOAD_U0 = (KIND == MID || KIND == MID_REBUILD);
+  static constexpr bool LOAD_U0 = (KIND == MID || KIND == MID_REBUILD || KIND == MID_NOACC || KIND == LAST_COMB);
   static constexpr bool LOAD_ACC = (KIND == MID || KIND == LAST);
+  static constexpr bool LOAD_Y23 = (KIND == LAST_COMB);   // the two earlier stage states Y2, Y3
   static constexpr bool WRITE_ACC = (KIND == FIRST || KIND == MID || KIND == MID_REBUILD);
-  static constexpr int NLOAD = (LOAD_U0 ? 1 : 0) + (LOAD_ACC ? 1 : 0);
-  // staging arrays of one u0/acc slot: array 0 = u0 on load (acc for LAST), y_out on store;
-  //                                    array 1 = acc on load (MID), acc_out on store
-  static constexpr int NARR = WRITE_ACC ? 2 : 1;
+  static constexpr int NLOAD = (LOAD_U0 ? 1 : 0) + (LOAD_ACC ? 1 : 0) + (LOAD_Y23 ? 2 : 0);
+  // staging arrays of one slot: array 0 = u0 on load (acc for LAST), y_out on store;
+  //                             array 1 = acc on load (MID) / Y2 (LAST_COMB), acc_out on store; array 2 = Y3
+  static constexpr int NARR = LOAD_Y23 ? 3 : (WRITE_ACC ? 2 : 1);
   static constexpr int ACC_LOAD_ARR = LOAD_U0 ? 1 : 0;
 };
 
@@ -124,7 +130,8 @@ struct StageSmem {
   static constexpr int NARR = KindTraits<KIND>::NARR;
   static constexpr uint32_t off_y = 0;
   static constexpr uint32_t off_ua = off_y + NY * YTILE;               // [NUA][NARR][PTILE]
-  static constexpr int XBUF = NSEG <= 8 ? 2 : 1;                        // copies of the flux exchange buffers
+  // copies of the flux exchange buffers (two when shared memory allows: lets neighbouring warps drift by one item)
+  static constexpr int XBUF = (NSEG <= 8 && NARR < 3) ? 2 : 1;
   static constexpr uint32_t XSZ = NSEG * 8u * VC * 8u, XBSZ = 8u * VC * 8u;
   static constexpr uint32_t off_x = off_ua + NUA * NARR * PTILE;       // [XBUF][NSEG][8][32] exchange (WENO)
   static constexpr uint32_t off_xb = off_x + (SCHEME == 1 ? XBUF * XSZ : 0u);  // [XBUF][8][32] boundary (WENO)
@@ -224,7 +231,8 @@ template <int SCHEME, int KIND, int TZ, int NSEG, int NY, int NUA>
 __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
     stage_kernel(const __grid_constant__ CUtensorMap tm_y,     // stage input with halo: box [8][TZ+2H][32]
                  const __grid_constant__ CUtensorMap tm_u0,    // U, rows 0..nz-1: box [8][TZ][32]
-                 const __grid_constant__ CUtensorMap tm_acc,   // RK accumulator (loaded and stored)
+                 const __grid_constant__ CUtensorMap tm_acc,   // RK accumulator (loaded and stored) / Y2 for LAST_COMB
+                 const __grid_constant__ CUtensorMap tm_y3,    // Y3 for LAST_COMB
                  const __grid_constant__ CUtensorMap tm_out,   // y_out, rows 0..nz-1
                  const StageParams p) {
   using SM = StageSmem<SCHEME, KIND, TZ, NSEG, NY, NUA>;
@@ -297,6 +305,10 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
           if constexpr (KT::LOAD_U0) tma_load_3d(dst, &tm_u0, b_full_ua + 8 * su, ch * VC, iz0, 0);
           if constexpr (KT::LOAD_ACC)
             tma_load_3d(dst + KT::ACC_LOAD_ARR * SM::PTILE, &tm_acc, b_full_ua + 8 * su, ch * VC, iz0, 0);
+          if constexpr (KT::LOAD_Y23) {
+            tma_load_3d(dst + SM::PTILE, &tm_acc, b_full_ua + 8 * su, ch * VC, iz0, 0);
+            tma_load_3d(dst + 2 * SM::PTILE, &tm_y3, b_full_ua + 8 * su, ch * VC, iz0, 0);
+          }
         } else {
           mbar_arrive(b_full_ua + 8 * su);   // nothing to load: the slot is free for staging
         }
@@ -470,10 +482,14 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
         const uint32_t cell = ((c * TZ + row) * VC) * 8;
         double u0v = yc[c], accb;
         if constexpr (KT::LOAD_U0) u0v = lds(Tu + cell);
-        if constexpr (KIND == FIRST || KIND == FIRST_LEAN) accb = yc[c];
+        if constexpr (KIND == FIRST || KIND == FIRST_LEAN || KIND == MID_NOACC) accb = yc[c];
         else if constexpr (KIND == MID_REBUILD) accb = fma(yc[c] - u0v, 1.0 / 3.0, u0v);  // u0 + (dt/6) k1
-        else accb = lds(Ta_in + cell);
-        const double base = (KIND == LAST) ? accb : u0v;
+        else if constexpr (KIND == LAST_COMB) {
+          // (Y2 + 2 Y3 + Y4 - U) / 3 = U + dt/6 (k1 + 2 k2 + 2 k3); Y4 is the stage input itself
+          const double y2 = lds(Tu + SM::PTILE + cell), y3 = lds(Tu + 2 * SM::PTILE + cell);
+          accb = (fma(2.0, y3, y2) + (yc[c] - u0v)) * (1.0 / 3.0);
+        } else accb = lds(Ta_in + cell);
+        const double base = (KIND == LAST || KIND == LAST_COMB) ? accb : u0v;
         const double o = fma(p.cy, k[c], base);
         sts(Tu + cell, o);
         if constexpr (KT::WRITE_ACC) sts(Ta_out + cell, fma(p.ca, k[c], accb));

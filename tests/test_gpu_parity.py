@@ -66,13 +66,13 @@ def test_one_step_random_state(B, R, scheme, nz, nv, variant):
 
 @pytest.mark.parametrize("variant", [0, 1])
 @pytest.mark.parametrize("scheme", [FD, FV])
-@pytest.mark.parametrize("lean", [False, True])
+@pytest.mark.parametrize("lean", [0, 1, 2])
 def test_20_steps_cfg0_shape(B, R, scheme, lean, variant):
     """BASELINE config 0 (fast conversion, 1024 x 16, dt = 0.4 dz), 20 steps, both schemes."""
     c = inputs.CONFIGS["cfg0"]
     st = inputs.config_state("cfg0")
     args = (c["nz"], c["nv"], c["L"], c["dt"], c["omega"], c["theta"], c["mu"], scheme)
-    got, ref, gm, rm, gd, rd = run_pair(B, R, args, st, 20, lean_acc=lean, variant=variant)
+    got, ref, gm, rm, gd, rd = run_pair(B, R, args, st, 20, rk_form=lean, variant=variant)
     assert np.max(np.abs(got - ref)) <= TOL20
     assert np.max(np.abs(gm - rm)) <= TOL20
     assert abs(gd["psurv_nu"] - rd["psurv_nu"]) <= 1e-12
