@@ -36,9 +36,9 @@ UNIT = "cell-updates/s"
 STAGE_BYTES = {0: [192, 320, 320, 192], 1: [128, 256, 320, 192], 2: [128, 192, 192, 320]}
 STAGE_KERNEL = {0: ["FIRST", "MID", "MID", "LAST"], 1: ["FIRST_LEAN", "MID_REBUILD", "MID", "LAST"],
                 2: ["FIRST_LEAN", "MID_NOACC", "MID_NOACC", "LAST_COMB"]}
-# dram__bytes_read.sum + dram__bytes_write.sum per MID-stage launch from the committed ncu capture
-# (profiles/), per workload; None until captured
-NCU_TRAFFIC_BYTES = {}
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant stage launch (RK stage 4, LAST_COMB) from the
+# committed ncu capture (profiles/r01_traffic_*.csv), per (workload, rk_form); None where not captured
+NCU_TRAFFIC_BYTES = {("cfg4", 2): 44279386880, ("cfg3", 2): 10752631296}   # profiles/r01_traffic_*.csv, RK stage 4
 
 
 def measured_peaks():

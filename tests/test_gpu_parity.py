@@ -221,3 +221,57 @@ def test_invariants_long_run_gpu(B):
         g.close()
         assert max(abs(x) for x in d["dM0"]) <= 1e-11 * nz
         assert np.isfinite(d["psurv_nu"]) and 0.0 < d["psurv_nu"] <= 1.0 + 1e-9
+
+
+# ---------------------------------------------------------------------------------------------------------
+# Full BASELINE sizes, in the launch configuration bench.py times.  The oracle cannot step 134 M cells, but one
+# RK4 step of a cell only depends on the cells within 4 stages x halo (<= 16 rows) of it, at all v.  So the
+# oracle, run on a z-window cut out of the SAME initial state (treated as a small periodic box), reproduces the
+# full-size result exactly on the rows that are farther than NSTEP*16 rows from the window's ends.
+def _window_parity(B, R, name, nsteps, windows, tol):
+    c = inputs.CONFIGS[name]
+    nz, nv = c["nz"], c["nv"]
+    dz = c["L"] / nz
+    st = inputs.config_state(name)
+    g = B.Cosenu(nz, nv, c["L"], c["dt"], c["omega"], c["theta"], c["mu"], c["scheme"])
+    g.set_state(st)
+    g.step(nsteps)
+    got = g.get_state()
+    gd = g.diagnostics()
+    g.close()
+    margin = 16 * nsteps + 4
+    worst = 0.0
+    for z0, w in windows:
+        rows = (np.arange(z0 - margin, z0 + w + margin)) % nz          # periodic wrap of the big grid
+        sub = np.ascontiguousarray(st[:, rows, :])
+        r = R.RefSim(len(rows), nv, len(rows) * dz, c["dt"], c["omega"], c["theta"], c["mu"], c["scheme"])
+        r.set_state(sub)
+        r.step(nsteps)
+        ref = r.get_state()[:, margin:margin + w, :]
+        r.close()
+        worst = max(worst, float(np.max(np.abs(got[:, rows[margin:margin + w], :] - ref))))
+    assert worst <= tol, worst
+    return gd
+
+
+def test_full_size_cfg2_windows(B, R):
+    c = inputs.CONFIGS["cfg2"]
+    _window_parity(B, R, "cfg2", 2, [(0, 8), (c["nz"] - 5, 10), (12345, 8), (c["nz"] // 2 - 3, 6)], 1e-13)
+
+
+def test_full_size_cfg3_windows(B, R):
+    c = inputs.CONFIGS["cfg3"]
+    _window_parity(B, R, "cfg3", 2, [(0, 8), (c["nz"] - 5, 10), (77777, 8)], 1e-13)
+
+
+def test_full_size_cfg4_windows(B, R):
+    import torch
+    free, _ = torch.cuda.mem_get_info()
+    if free < 40e9:
+        pytest.skip("needs 35 GB of device memory")
+    c = inputs.CONFIGS["cfg4"]
+    d = _window_parity(B, R, "cfg4", 1, [(0, 6), (c["nz"] - 3, 6), (200001, 6)], 1e-13)
+    # invariants at full size: trace per cell, lepton number along B (omega != 0: only B.M0 is conserved)
+    assert d["trace_dev_max"] <= 1e-12
+    s2, c2 = np.sin(2 * c["theta"]), np.cos(2 * c["theta"])
+    assert abs(s2 * d["dM0"][0] - c2 * d["dM0"][2]) <= 1e-9 * c["nz"]
