@@ -93,6 +93,22 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def max_over_ranks(x, device="cuda"):
+    """Max of a per-rank scalar over all ranks (the job is as slow as its slowest rank)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(x)
+    t = torch.tensor([float(x)], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(cells, steps, world, ms):
+    """Whole-job aggregate: every rank advances its own `cells` grid by `steps` steps (weak scaling)."""
+    return world * cells * steps / (ms * 1e-3)
+
+
 def workload(name):
     from paper_2203_12866_b200 import inputs
     c = dict(inputs.CONFIGS[name])
@@ -102,7 +118,6 @@ def workload(name):
 
 def oracle_sample(c, target_s=15.0, max_nz=4096):
     """Time the oracle, as it stands, on a z-reduced sample of workload c (same nv, scheme, physics)."""
-    import numpy as np
     from oracle import cosenu_ref as R
     from paper_2203_12866_b200 import inputs
     nz = min(c["nz"], max_nz)
@@ -124,9 +139,6 @@ def run_reference(args):
     if rank != 0:
         return
     c = workload(args.workload)
-    per_step_target = 4.0
-    vals = []
-    import numpy as np
     from oracle import cosenu_ref as R
     from paper_2203_12866_b200 import inputs
     nz = min(c["nz"], 2048)
@@ -207,11 +219,8 @@ def run_ours(args):
     stage_ms, nst = sim.stage_times()
     sim.set_option(B.OPT_STAGE_TIMING, 0)
     clocks = sampler.stop() if rank == 0 else None
-    if world > 1:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * cells * args.steps / (ms * 1e-3)
+    ms = max_over_ranks(ms)
+    value = whole_job_value(cells, args.steps, world, ms)
 
     # ---- invariants at the bench size (properties that hold at any size)
     d1 = sim.diagnostics()
@@ -229,10 +238,7 @@ def run_ours(args):
         sim.get_state(host)       # synchronises
     barrier()
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = max_over_ranks(e2e_s)
     state_bytes = 8 * cells * 8
     e2e = {"value": world * cells * ne2e / e2e_s, "unit": UNIT, "h2d_bytes_per_step": state_bytes,
            "d2h_bytes_per_step": state_bytes, "steps": ne2e,

@@ -83,3 +83,59 @@ def test_kernel_fd_formula_matches_definition_and_is_exact_on_constants(libs):
         assert abs(a - b) <= 1e-14 / dz
     u = np.full(5, 0.7331)
     assert probe.cosenu_probe_fd4_ko3(u.ctypes.data_as(dp), 0.9, 1.0, 0.1) == 0.0
+
+
+def test_kernel_weno_form_against_exact_rational_algorithm1(libs):
+    """Algorithm 1 in exact rational arithmetic is the judge between the two fp64 evaluation
+    orders: the oracle's literal Eq. (A.3) polynomials and the kernels' difference form.  Both must agree with it;
+    for nearly constant O(1) data the literal form loses digits, the difference form must not."""
+    from fractions import Fraction as F
+    from oracle import cosenu_ref as R
+    _, probe = libs
+    dp = C.POINTER(C.c_double)
+    probe.cosenu_probe_weno7_face.restype = C.c_double
+    probe.cosenu_probe_weno7_face.argtypes = [dp, C.c_double, C.c_double]
+    probe.cosenu_probe_weno7_face2.restype = None
+    probe.cosenu_probe_weno7_face2.argtypes = [dp, C.c_double, C.c_double, dp]
+
+    def exact(f, eps):
+        m3, m2, m1, c, p1, p2, p3 = [F(x) for x in f]
+        fh = [(3 * c + 13 * p1 - 5 * p2 + p3) / 12, (-m1 + 7 * c + 7 * p1 - p2) / 12,
+              (m2 - 5 * m1 + 13 * c + 3 * p1) / 12, (-3 * m3 + 13 * m2 - 23 * m1 + 25 * c) / 12]
+        si = [c * (2107 * c - 9402 * p1 + 7042 * p2 - 1854 * p3) + p1 * (11003 * p1 - 17246 * p2 + 4642 * p3)
+              + p2 * (7043 * p2 - 3882 * p3) + 547 * p3 * p3,
+              m1 * (547 * m1 - 2522 * c + 1922 * p1 - 494 * p2) + c * (3443 * c - 5966 * p1 + 1602 * p2)
+              + p1 * (2843 * p1 - 1642 * p2) + 267 * p2 * p2,
+              m2 * (267 * m2 - 1642 * m1 + 1602 * c - 494 * p1) + m1 * (2843 * m1 - 5966 * c + 1922 * p1)
+              + c * (3443 * c - 2522 * p1) + 547 * p1 * p1,
+              m3 * (547 * m3 - 3882 * m2 + 4642 * m1 - 1854 * c) + m2 * (7043 * m2 - 17246 * m1 + 7042 * c)
+              + m1 * (11003 * m1 - 9402 * c) + 2107 * c * c]
+        d = [F(4, 35), F(18, 35), F(12, 35), F(1, 35)]
+        w = [d[r] / (si[r] + F(eps)) ** 2 for r in range(4)]
+        return sum(w[r] * fh[r] for r in range(4)) / sum(w)
+
+    rng = np.random.default_rng(7)
+    worst_kernel, worst_oracle = 0.0, 0.0
+    for trial in range(300):
+        kind = trial % 3
+        if kind == 0:
+            u = rng.standard_normal(8)
+        elif kind == 1:
+            u = 1.0 + 1e-3 * rng.standard_normal(8)          # nearly constant O(1): the cancellation case
+        else:
+            u = np.sin(0.25 * np.arange(8) + rng.uniform(0, 6))
+        v, eps = float(rng.uniform(0.05, 1.0)), 1e-6
+        f = [v * x for x in u]                                # Algorithm 1 acts on f = v u (reading A8)
+        ex = exact(f[:7], eps)
+        a = probe.cosenu_probe_weno7_face(u[:7].copy().ctypes.data_as(dp), v, eps)
+        o = R.weno7_face(np.array(f[:7]), eps)
+        scale = max(abs(x) for x in f)
+        ek, eo = abs(F(a) - ex) / F(scale), abs(F(o) - ex) / F(scale)
+        worst_kernel, worst_oracle = max(worst_kernel, float(ek)), max(worst_oracle, float(eo))
+        # the paired routine gives the same two interfaces as two single calls
+        out = np.empty(2)
+        probe.cosenu_probe_weno7_face2(u.ctypes.data_as(dp), v, eps, out.ctypes.data_as(dp))
+        b = probe.cosenu_probe_weno7_face(u[1:8].copy().ctypes.data_as(dp), v, eps)
+        assert abs(out[0] - a) <= 4e-16 * scale and abs(out[1] - b) <= 4e-16 * scale
+    assert worst_kernel <= 2e-15, worst_kernel     # the kernels' form is accurate to a few ulp everywhere
+    assert worst_oracle <= 5e-11, worst_oracle     # the literal form is right too, up to its cancellation noise
