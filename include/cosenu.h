@@ -60,7 +60,7 @@ enum {
                               default 2 */
   COSENU_OPT_STAGE_TIMING = 4, /* 1: bracket every stage launch with CUDA events on the handle's stream
                               (read with cosenu_stage_times); default 0 */
-  COSENU_OPT_VARIANT = 5   /* kernel shape: 0 = 16 compute warps x 1 row (default), 1 = 8 compute warps x 2 rows;
+  COSENU_OPT_VARIANT = 5   /* kernel shape: 0 = 8 compute warps x 2 rows (default), 1 = 16 compute warps x 1 row;
                               same arithmetic per cell, different summation grouping of the moments only */
 };
 

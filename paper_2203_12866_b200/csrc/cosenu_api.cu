@@ -190,11 +190,11 @@ int launch_kind(cosenu* h, int kind, const CUtensorMap& map, const CUtensorMap& 
 int launch_stage(cosenu* h, int kind, const CUtensorMap& map, const CUtensorMap& omap, const CUtensorMap& a1,
                  const CUtensorMap& a2, const StageParams& p) {
   if (h->scheme == COSENU_FD4_KO3) {
-    if (h->variant == 1) return launch_kind<0, TZ_ALL, 8, 2, 2>(h, kind, map, omap, a1, a2, p);
-    return launch_kind<0, TZ_ALL, 16, 2, 2>(h, kind, map, omap, a1, a2, p);
+    if (h->variant == 1) return launch_kind<0, TZ_ALL, 16, 2, 2>(h, kind, map, omap, a1, a2, p);
+    return launch_kind<0, TZ_ALL, 8, 2, 2>(h, kind, map, omap, a1, a2, p);
   }
-  if (h->variant == 1) return launch_kind<1, TZ_ALL, 8, 2, 1>(h, kind, map, omap, a1, a2, p);
-  return launch_kind<1, TZ_ALL, 16, 2, 1>(h, kind, map, omap, a1, a2, p);
+  if (h->variant == 1) return launch_kind<1, TZ_ALL, 16, 2, 1>(h, kind, map, omap, a1, a2, p);
+  return launch_kind<1, TZ_ALL, 8, 2, 1>(h, kind, map, omap, a1, a2, p);
 }
 
 StageParams base_params(const cosenu* h) {
