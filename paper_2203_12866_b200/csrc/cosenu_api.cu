@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <set>
 #include <string>
 #include <vector>
 
@@ -64,6 +65,8 @@ struct cosenu {
   // stage timing
   std::vector<cudaEvent_t> ev_pool; size_t ev_used = 0;
   double stage_ms[4] = {0, 0, 0, 0}; int64_t stage_n = 0;
+
+  std::set<const void*> configured;   // stage kernels whose shared-memory attribute is set on this device
 
   std::string err;
 };
@@ -160,10 +163,11 @@ int launch_one(cosenu* h, const CUtensorMap& map, const CUtensorMap& omap, const
   auto kern = stage_kernel<SCHEME, KIND, TZ, NSEG, NY, NUA>;
   constexpr size_t smem = StageSmem<SCHEME, KIND, TZ, NSEG, NY, NUA>::bytes;
   static_assert(smem <= 232448, "over the 227 KB shared-memory limit of a CTA");
-  static bool configured = false;  // per instantiation
-  if (!configured) {
+  // the opt-in to > 48 KB of dynamic shared memory is per function and per device: remember it per handle
+  const void* key = reinterpret_cast<const void*>(kern);
+  if (h->configured.find(key) == h->configured.end()) {
     CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    configured = true;
+    h->configured.insert(key);
   }
   const long long ntiles = (h->nz + TZ - 1) / TZ;
   const unsigned grid = (unsigned)(ntiles < h->num_sms ? ntiles : h->num_sms);   // persistent: one CTA per SM
@@ -178,7 +182,8 @@ int launch_kind(cosenu* h, int kind, const CUtensorMap& map, const CUtensorMap& 
                 const CUtensorMap& a2, const StageParams& p) {
   switch (kind) {
     case FIRST: return launch_one<SCHEME, FIRST, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
-    case FIRST_LEAN: return launch_one<SCHEME, FIRST_LEAN, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
+    // stage 1 of the lean forms loads nothing but the stage input: a deeper input ring keeps enough bytes in flight
+    case FIRST_LEAN: return launch_one<SCHEME, FIRST_LEAN, TZ, NSEG, (SCHEME == 0 ? 4 : NY), NUA>(h, map, omap, a1, a2, p);
     case MID: return launch_one<SCHEME, MID, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
     case MID_REBUILD: return launch_one<SCHEME, MID_REBUILD, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
     case LAST: return launch_one<SCHEME, LAST, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
