@@ -1,0 +1,121 @@
+"""The CUDA path against what the paper and the mathematics fix, WITHOUT the oracle in between: the discrete
+closed form of the linear (mu = 0) system (this is BASELINE config 1's check at full
+length), Eq. (17) with the printed 0.076, and the convergence orders of PAPER.md:164."""
+import numpy as np
+import pytest
+
+from paper_2203_12866_b200 import analysis, inputs
+from test_oracle_pins import fd_ko_symbol, linear_closed_form, weno_linear_symbol
+
+pytestmark = pytest.mark.gpu
+FD, FV = 0, 1
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2203_12866_b200 import binding
+    return binding
+
+
+def test_config1_full_run_discrete_closed_form(B):
+    """BASELINE config 1 (vacuum only, 4096 x 64, 2000 steps): exact advection shift + per-mode precession of the
+    DISCRETE scheme (circulant FD4+KO3 symbol x rotation, RK4 stability polynomial to the 2000th power)."""
+    c = inputs.CONFIGS["cfg1"]
+    st = inputs.config_state("cfg1")
+    g = B.Cosenu(c["nz"], c["nv"], c["L"], c["dt"], c["omega"], c["theta"], c["mu"], c["scheme"])
+    g.set_state(st)
+    g.step(c["steps"])
+    got = g.get_state()
+    g.close()
+    want = linear_closed_form(st, c["steps"], c["dt"], c["omega"], c["theta"],
+                              fd_ko_symbol(c["nz"], c["nv"], c["L"] / c["nz"], 0.1))
+    assert np.max(np.abs(got - want)) <= 2e-12
+    # the loose, continuous version: rho_ee of every beam is the initial modulation shifted by v t (KO damps the
+    # k = 4 mode by < 1e-9 here), up to the precession that mixes ee and xx with amplitude sin^2(2 theta)
+    tr = got[0] + got[1]
+    t = c["steps"] * c["dt"]
+    z = np.arange(c["nz"]) * (c["L"] / c["nz"])
+    v = inputs.v_grid(c["nv"])
+    gnu, _ = inputs.angular_distributions(c["nv"])
+    shifted = gnu[None, :] * (1.0 + 0.1 * np.sin(2 * np.pi * 4 * (z[:, None] - v[None, :] * t) / c["L"]))
+    assert np.max(np.abs(tr - shifted)) <= 1e-6
+
+
+def test_weno_linear_limit_closed_form_gpu(B):
+    nz, nv, dt, nsteps = 256, 40, 0.4, 300
+    st = inputs.random_state(nz, nv, 79)
+    g = B.Cosenu(nz, nv, float(nz), dt, 1.0, 0.1, 0.0, FV, weno_eps=1e30)
+    g.set_state(st); g.step(nsteps)
+    want = linear_closed_form(st, nsteps, dt, 1.0, 0.1, weno_linear_symbol(nz, nv, 1.0))
+    assert np.max(np.abs(g.get_state() - want)) <= 2e-13
+    g.close()
+
+
+@pytest.mark.parametrize("scheme", [FD, FV])
+def test_eq17_vacuum_solution_gpu(B, golden, scheme):
+    gv = golden("paper_values.txt")
+    om = float(gv["omega_vac"]); th = np.deg2rad(float(gv["theta_vac_deg"]))
+    nz, nv, dt = 64, 4, 0.05
+    sim = B.Cosenu(nz, nv, 64.0, dt, om, th, 0.0, scheme)
+    st = np.zeros((8, nz, nv)); st[0] = 1.0; st[4] = 0.7
+    sim.set_state(st)
+    s2, c2 = np.sin(2 * th), np.cos(2 * th)
+    minee = 1.0
+    for n in range(1, 281):
+        sim.step(5)
+        t = 5 * n * dt
+        ss = np.sin(om * t / 2) ** 2
+        want = [1 - s2 * s2 * ss, s2 * s2 * ss, -s2 * c2 * ss, 0.5 * s2 * np.sin(om * t)]
+        if n % 20 == 0:
+            y = sim.get_state()
+            for c in range(4):
+                assert np.allclose(y[c], want[c], rtol=0, atol=2e-10), (n, c)
+                assert np.allclose(y[4 + c], 0.7 * want[c], rtol=0, atol=2e-10), (n, c)
+        d = sim.diagnostics()
+        assert abs(d["psurv_nu"] - want[0]) < 2e-10 and abs(d["psurv_nubar"] - want[0]) < 2e-10
+        minee = min(minee, d["psurv_nu"])
+    sim.close()
+    # the printed minimum of <rho_ee>, to its three printed decimals
+    assert abs(minee - float(gv["min_rho_ee_theta37"])) < 5e-4
+
+
+def _advection_error_gpu(B, scheme, nz, eps_ko=None, weno_eps=None, T=2.0):
+    nv, L = 2, 2 * np.pi
+    dz = L / nz
+    nsteps = int(np.ceil(T / (0.02 * dz))); dt = T / nsteps
+    sim = B.Cosenu(nz, nv, L, dt, 0.0, 0.0, 0.0, scheme, eps_ko=eps_ko, weno_eps=weno_eps)
+    zl = np.arange(nz) * dz
+    if scheme == FV:
+        f0 = lambda x: (np.cos(x) - np.cos(x + dz)) / dz     # cell averages of sin (reading A13)
+    else:
+        f0 = np.sin
+    st = np.zeros((8, nz, nv)); st[0] = f0(zl)[:, None]
+    sim.set_state(st); sim.step(nsteps)
+    y = sim.get_state()[0]
+    sim.close()
+    v = inputs.v_grid(nv)
+    return max(analysis.e2_norm(y[:, j], f0(zl - v[j] * T)) for j in range(nv))
+
+
+def test_convergence_orders_gpu(B, golden):
+    gv = golden("paper_values.txt")
+    e = [_advection_error_gpu(B, FD, n, eps_ko=0.0) for n in (16, 32)]
+    assert abs(analysis.order_of_convergence(*e) - float(gv["order_fd4"])) < 0.25
+    e = [_advection_error_gpu(B, FV, n, weno_eps=1e30) for n in (16, 32)]
+    assert abs(analysis.order_of_convergence(*e) - float(gv["order_weno7"])) < 0.4
+    e = [_advection_error_gpu(B, FV, n, weno_eps=1e-6) for n in (16, 32)]
+    assert 5.0 < analysis.order_of_convergence(*e) < 8.5
+
+
+def test_conserved_quantity_scan_improves_with_resolution(B):
+    """Fig. 8, qualitatively: the |P| deviations of the WENO7 run shrink when dz shrinks at
+    fixed physical length and C_CFL; M0 stays conserved to rounding at every resolution."""
+    rows = analysis.conserved_quantity_scan(
+        lambda nz, L, dt: B.Cosenu(nz, 32, L, dt, 0.0, 0.0, 1.0, FV), [256, 512, 1024], t_end=300.0, L=256.0,
+        seed=3, pert_amp=1e-3)
+    assert rows[2]["dP_max"] < rows[1]["dP_max"] < rows[0]["dP_max"]
+    assert all(r["dM0_max"] <= 1e-11 for r in rows)
+    assert analysis.kappa(rows[0]["dP_avg"], rows[1]["dP_avg"], rows[2]["dP_avg"]) > 1.0
