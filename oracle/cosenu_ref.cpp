@@ -26,9 +26,10 @@ struct cosenu_ref {
   double L, dt, omega, theta, mu; int scheme;
   double eps_ko = 0.1;      // PAPER.md:164 "KO3 with eps_KO = 0.1"
   double weno_eps = 1e-6;   // PAPER.md:145 "typical value ~1e-6"
-  int advect = 1; int threads = 0;
+  int advect = 1; int threads = 0; int quad = 0;
   double dz, dv;
-  std::vector<double> v;    // bin centres
+  std::vector<double> v;    // beam velocities: bin centres or vertex-centred points
+  std::vector<double> wq;   // quadrature weights in units of dv: int f dv ~ dv * sum_j wq_j f(v_j)
   std::vector<double> y;    // current state, canonical layout [8][nz][nv]
   bool have_state = false;
   double t = 0; int64_t step = 0;
@@ -42,6 +43,24 @@ struct cosenu_ref {
 static std::string g_err;  // last error of a failed create
 
 static inline int64_t wrap(int64_t i, int64_t n) { return ((i % n) + n) % n; }
+
+// v-grid and quadrature weights (readings A1 and section 3.1 of the paper)
+static void build_vgrid(cosenu_ref* h) {
+  const int nv = h->nv;
+  h->v.resize(nv); h->wq.assign(nv, 1.0);
+  if (h->quad == 0) {             // bins [v_j, v_j + dv] represented by their centres; simple Riemann sum
+    h->dv = 2.0 / (double)nv;
+    for (int j = 0; j < nv; ++j) h->v[j] = -1.0 + (j + 0.5) * h->dv;
+  } else {                        // fixed-width vertex-centred points over [-1, 1]
+    h->dv = 2.0 / (double)(nv - 1);
+    for (int j = 0; j < nv; ++j) h->v[j] = -1.0 + (double)j * h->dv;
+    if (h->quad == 1) {           // trapezoid rule
+      h->wq[0] = h->wq[nv - 1] = 0.5;
+    } else {                      // Simpson's rule: (1, 4, 2, 4, ..., 4, 1)/3
+      for (int j = 0; j < nv; ++j) h->wq[j] = (j == 0 || j == nv - 1) ? 1.0 / 3.0 : ((j & 1) ? 4.0 / 3.0 : 2.0 / 3.0);
+    }
+  }
+}
 static inline size_t idx(const cosenu_ref* h, int c, int64_t iz, int iv) {
   return ((size_t)c * h->nz + iz) * h->nv + iv;
 }
@@ -104,8 +123,8 @@ static void moments(const cosenu_ref* h, const double* y, double* M /*[6][nz]*/)
       double Dd = (y[idx(h, 0, i, j)] - y[idx(h, 1, i, j)]) - (y[idx(h, 4, i, j)] - y[idx(h, 5, i, j)]);
       double Dr = y[idx(h, 2, i, j)] - y[idx(h, 6, i, j)];
       double Di = y[idx(h, 3, i, j)] + y[idx(h, 7, i, j)];  // conj of rho_bar flips Im only
-      long double vj = h->v[j];
-      s[0] += Dd; s[1] += vj * Dd; s[2] += Dr; s[3] += vj * Dr; s[4] += Di; s[5] += vj * Di;
+      const long double vj = h->v[j], w = h->wq[j];
+      s[0] += w * Dd; s[1] += w * (vj * Dd); s[2] += w * Dr; s[3] += w * (vj * Dr); s[4] += w * Di; s[5] += w * (vj * Di);
     }
     for (int m = 0; m < 6; ++m) M[(size_t)m * nz + i] = (double)(s[m] * (long double)h->dv);
   }
@@ -224,7 +243,8 @@ static void m0_vector(const cosenu_ref* h, const double* y, double M0[3]) {
       const double Dd = (y[idx(h, 0, i, j)] - y[idx(h, 1, i, j)]) - (y[idx(h, 4, i, j)] - y[idx(h, 5, i, j)]);
       const double Dr = y[idx(h, 2, i, j)] - y[idx(h, 6, i, j)];
       const double Di = y[idx(h, 3, i, j)] + y[idx(h, 7, i, j)];
-      s[0] += 2.0 * Dr; s[1] += -2.0 * Di; s[2] += Dd;  // P = (2 Re, -2 Im, ee - xx)
+      const long double w = h->wq[j];
+      s[0] += w * (2.0 * Dr); s[1] += w * (-2.0 * Di); s[2] += w * Dd;  // P = (2 Re, -2 Im, ee - xx)
     }
   for (int m = 0; m < 3; ++m) M0[m] = (double)(s[m] * (long double)(h->dz * h->dv));
 }
@@ -238,7 +258,7 @@ static void take_references(cosenu_ref* h) {
       for (int64_t i = 0; i < h->nz; ++i) {
         sp += plen(h->y.data(), h, s, i, j);
         s0 += h->y[idx(h, 4 * s, i, j)] + h->y[idx(h, 4 * s + 1, i, j)];
-        see += h->y[idx(h, 4 * s, i, j)];
+        see += (long double)h->wq[j] * h->y[idx(h, 4 * s, i, j)];
       }
       h->Pref[s][j] = (double)(sp / h->nz); h->P0ref[s][j] = (double)(s0 / h->nz);
     }
@@ -257,9 +277,8 @@ extern "C" cosenu_ref_t* cosenu_ref_create(int64_t nz, int32_t nv, double L, dou
   cosenu_ref* h = new (std::nothrow) cosenu_ref();
   if (!h) { g_err = "out of memory"; return nullptr; }
   h->nz = nz; h->nv = nv; h->L = L; h->dt = dt; h->omega = omega; h->theta = theta; h->mu = mu; h->scheme = scheme;
-  h->dz = L / (double)nz; h->dv = 2.0 / (double)nv;
-  h->v.resize(nv);
-  for (int j = 0; j < nv; ++j) h->v[j] = -1.0 + (j + 0.5) * h->dv;  // bin centres
+  h->dz = L / (double)nz;
+  build_vgrid(h);
   try { h->y.assign(8 * (size_t)nz * nv, 0.0); } catch (...) { delete h; g_err = "out of memory"; return nullptr; }
   return h;
 }
@@ -271,6 +290,9 @@ extern "C" int cosenu_ref_set_option(cosenu_ref_t* h, int key, double value) {
     case COSENU_REF_OPT_WENO_EPS: if (!(value > 0)) break; h->weno_eps = value; return COSENU_REF_OK;
     case COSENU_REF_OPT_ADVECT: h->advect = value != 0; return COSENU_REF_OK;
     case COSENU_REF_OPT_THREADS: if (value < 0) break; h->threads = (int)value; return COSENU_REF_OK;
+    case COSENU_REF_OPT_QUADRATURE:
+      if ((value != 0 && value != 1 && value != 2) || h->have_state || (value == 2 && (h->nv % 2 == 0 || h->nv < 3))) break;
+      h->quad = (int)value; build_vgrid(h); return COSENU_REF_OK;
   }
   h->err = "cosenu_ref_set_option: bad key or value"; return COSENU_REF_EINVAL;
 }
@@ -296,7 +318,7 @@ extern "C" int cosenu_ref_init(cosenu_ref_t* h, uint64_t seed, double sigma_nu, 
   for (int j = 0; j < nv; ++j) {
     g[j] = std::exp(-(h->v[j] - 1.0) * (h->v[j] - 1.0) / (2.0 * sigma_nu * sigma_nu));
     gb[j] = std::exp(-(h->v[j] - 1.0) * (h->v[j] - 1.0) / (2.0 * sigma_nubar * sigma_nubar));
-    sg += g[j]; sgb += gb[j];
+    sg += h->wq[j] * g[j]; sgb += h->wq[j] * gb[j];
   }
   for (int j = 0; j < nv; ++j) { g[j] = g[j] / (sg * h->dv); gb[j] = alpha * (gb[j] / (sgb * h->dv)); }
   const double two_pi = 6.283185307179586476925286766559;
@@ -379,10 +401,11 @@ extern "C" int cosenu_ref_diagnostics(cosenu_ref_t* h, cosenu_ref_diag_t* d) {
   for (int s = 0; s < 2; ++s)
     for (int64_t i = 0; i < h->nz; ++i)
       for (int j = 0; j < h->nv; ++j) {
-        see[s] += y[idx(h, 4 * s, i, j)];
+        const long double w = h->wq[j];
+        see[s] += w * y[idx(h, 4 * s, i, j)];
         const double P = plen(y, h, s, i, j), Pr = h->Pref[s][j];
         if (Pr > 0) { const double dp = std::fabs(P / Pr - 1.0); if (dp > dpmax) dpmax = dp; }  // Eq. (22)
-        if (s == 0) { num += std::fabs(P - Pr); den += Pr; }                                    // Eq. (23)
+        if (s == 0) { num += w * std::fabs(P - Pr); den += w * Pr; }                                    // Eq. (23)
         const double tr = std::fabs(y[idx(h, 4 * s, i, j)] + y[idx(h, 4 * s + 1, i, j)] - h->P0ref[s][j]);
         if (tr > trmax) trmax = tr;
         const double ex = std::hypot(y[idx(h, 4 * s + 2, i, j)], y[idx(h, 4 * s + 3, i, j)]);

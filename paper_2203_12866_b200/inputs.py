@@ -30,29 +30,51 @@ def splitmix64_uniform(seed: int, n: int) -> np.ndarray:
     return (z >> np.uint64(11)).astype(np.float64) * (1.0 / 9007199254740992.0)
 
 
-def v_grid(nv: int) -> np.ndarray:
-    return -1.0 + (np.arange(nv) + 0.5) * (2.0 / nv)
+MIDPOINT, TRAPEZOID, SIMPSON = 0, 1, 2
 
 
-def angular_distributions(nv: int, sigma_nu=0.6, sigma_nubar=0.5, alpha=0.9):
-    v = v_grid(nv)
-    dv = 2.0 / nv
+def v_grid(nv: int, quadrature: int = MIDPOINT) -> np.ndarray:
+    """Beam velocities: bin centres or, for the trapezoid / Simpson variants of the FD
+    implementation, fixed-width vertex-centred points over [-1, 1]."""
+    if quadrature == MIDPOINT:
+        return -1.0 + (np.arange(nv) + 0.5) * (2.0 / nv)
+    return -1.0 + np.arange(nv) * (2.0 / (nv - 1))
+
+
+def v_weights(nv: int, quadrature: int = MIDPOINT):
+    """(dv, w): int f dv ~ dv * sum_j w_j f(v_j)."""
+    if quadrature == MIDPOINT:
+        return 2.0 / nv, np.ones(nv)
+    w = np.ones(nv)
+    if quadrature == TRAPEZOID:
+        w[0] = w[-1] = 0.5
+    else:
+        assert nv % 2 == 1 and nv >= 3
+        w[:] = np.where(np.arange(nv) % 2 == 1, 4.0 / 3.0, 2.0 / 3.0)
+        w[0] = w[-1] = 1.0 / 3.0
+    return 2.0 / (nv - 1), w
+
+
+def angular_distributions(nv: int, sigma_nu=0.6, sigma_nubar=0.5, alpha=0.9, quadrature: int = MIDPOINT):
+    v = v_grid(nv, quadrature)
+    dv, w = v_weights(nv, quadrature)
     g = np.exp(-(v - 1.0) * (v - 1.0) / (2.0 * sigma_nu * sigma_nu))
     gb = np.exp(-(v - 1.0) * (v - 1.0) / (2.0 * sigma_nubar * sigma_nubar))
     # sequential sums (same order as the C generators) so all three agree to the last bit
     sg = 0.0
     sgb = 0.0
     for j in range(nv):
-        sg += g[j]
-        sgb += gb[j]
+        sg += w[j] * g[j]
+        sgb += w[j] * gb[j]
     g = g / (sg * dv)
     gb = alpha * (gb / (sgb * dv))
     return g, gb
 
 
-def fast_conversion_state(nz, nv, seed, pert_amp=1e-6, sigma_nu=0.6, sigma_nubar=0.5, alpha=0.9):
+def fast_conversion_state(nz, nv, seed, pert_amp=1e-6, sigma_nu=0.6, sigma_nubar=0.5, alpha=0.9,
+                          quadrature: int = MIDPOINT):
     """BASELINE configs 0, 2, 3, 4: z-homogeneous g, g_bar with a seeded random-phase rho_ex."""
-    g, gb = angular_distributions(nv, sigma_nu, sigma_nubar, alpha)
+    g, gb = angular_distributions(nv, sigma_nu, sigma_nubar, alpha, quadrature)
     phi = 2.0 * np.pi * splitmix64_uniform(seed, nz)
     pr = pert_amp * np.cos(phi)
     pi = pert_amp * np.sin(phi)

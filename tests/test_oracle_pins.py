@@ -378,10 +378,10 @@ def test_P8_uniform_state_has_zero_advection(scheme):
 
 
 # ----------------------------------------------------------------------------- P9: brute force
-def _brute_force_commutator(st, omega, theta, mu):
+def _brute_force_commutator(st, omega, theta, mu, quadrature=0):
     """Eq. (1), (3a), (3b) with 2x2 complex matrices and the direct double sum."""
     _, nz, nv = st.shape
-    v = inputs.v_grid(nv); dv = 2.0 / nv
+    v = inputs.v_grid(nv, quadrature); dv, wq = inputs.v_weights(nv, quadrature)
     Hv = 0.5 * omega * np.array([[-np.cos(2 * theta), np.sin(2 * theta)], [np.sin(2 * theta), np.cos(2 * theta)]])
     out = np.zeros_like(st)
     for i in range(nz):
@@ -392,7 +392,7 @@ def _brute_force_commutator(st, omega, theta, mu):
         for j in range(nv):
             H = Hv.astype(complex).copy(); Hb = Hv.astype(complex).copy()
             for jp in range(nv):
-                w = dv * (1 - v[j] * v[jp])
+                w = dv * wq[jp] * (1 - v[j] * v[jp])
                 H += mu * w * (rho[jp] - np.conj(rhob[jp]))      # Eq. (3a); alpha folded into rho_bar
                 Hb -= mu * w * (np.conj(rho[jp]) - rhob[jp])     # Eq. (3b)
             d = -1j * (H @ rho[j] - rho[j] @ H)
@@ -525,3 +525,62 @@ def test_abi_argument_validation():
     assert L.cosenu_ref_step(sim.h, 1) == 4  # ESTATE before init
     with pytest.raises(RuntimeError):
         sim.set_option(99, 1.0)
+
+
+# ----------------------------------------------------------------------------- section 3.1 quadrature variants
+@pytest.mark.parametrize("quad,nv", [(1, 2), (1, 9), (1, 16), (2, 3), (2, 9), (2, 17)])
+def test_quadrature_variants_grid_and_polynomial_exactness(quad, nv):
+    """fixed-width vertex-centred points over [-1,1] with the trapezoid rule (2nd order) or
+    Simpson's rule (4th order).  Closed forms: the trapezoid rule is exact for linear integrands and, by
+    Euler-Maclaurin, off by exactly (h^2/12)[f'(1) - f'(-1)] for cubics; Simpson's rule is exact for cubics."""
+    nz = 16
+    sim = R.RefSim(nz, nv, 16.0, 0.1, 0.0, 0.0, 1.0, FD, quadrature=quad)
+    v = inputs.v_grid(nv, quad)
+    h = 2.0 / (nv - 1)
+    assert v[0] == -1.0 and abs(v[-1] - 1.0) < 1e-15 and np.allclose(np.diff(v), h)
+    a, b, c, d = 0.7, -0.3, 0.45, 0.9
+    p = a + b * v + c * v ** 2 + d * v ** 3
+    st = np.zeros((8, nz, nv)); st[0] = p[None, :]          # Dd = p(v), everything else 0
+    M = sim.moments(st)
+    I0 = 2 * a + 2 * c / 3                                   # int_{-1}^{1} p dv
+    I1 = 2 * b / 3 + 2 * d / 5                               # int v p dv
+    if quad == 2:
+        assert np.allclose(M[0], I0, atol=1e-14)             # cubic: exact
+        lin = np.zeros((8, nz, nv)); lin[0] = (a + b * v + c * v ** 2)[None, :]
+        assert np.allclose(sim.moments(lin)[1], 2 * b / 3, atol=1e-14)   # v * quadratic = cubic: exact
+    else:
+        # f = p: f' = b + 2 c v + 3 d v^2  ->  f'(1) - f'(-1) = 4 c
+        assert np.allclose(M[0], I0 + h * h / 12 * 4 * c, atol=1e-14)
+        # f = v p (quartic): check only its cubic part, d = 0
+        st2 = np.zeros((8, nz, nv)); st2[0] = (a + b * v + c * v ** 2)[None, :]
+        # (v p)' = a + 2 b v + 3 c v^2 -> difference 4 b
+        assert np.allclose(sim.moments(st2)[1], 2 * b / 3 + h * h / 12 * 4 * b, atol=1e-14)
+    assert np.abs(M[2:]).max() == 0.0
+
+
+@pytest.mark.parametrize("quad,nv", [(1, 4), (2, 5)])
+def test_quadrature_variants_commutator_brute_force_and_invariants(quad, nv):
+    nz = 16
+    st = inputs.random_state(nz, nv, 300 + nv)
+    sim = R.RefSim(nz, nv, 16.0, 0.1, 0.4, 0.3, 2.5, FD, advect=False, quadrature=quad)
+    assert np.abs(sim.rhs(st) - _brute_force_commutator(st, 0.4, 0.3, 2.5, quad)).max() < 2e-13
+    # M0 conservation (Eq. 19) holds for any quadrature used consistently in H and in M0 (P10)
+    run = R.RefSim(nz, nv, 16.0, 0.05, 0.0, 0.0, 1.0, FD, quadrature=quad)
+    run.set_state(st); run.step(100)
+    d = run.diagnostics()
+    assert max(abs(x) for x in d["dM0"]) < 1e-12
+    # init: the discrete normalisation uses the same rule
+    ini = R.RefSim(32, nv, 32.0, 0.1, 0.0, 0.0, 1.0, FD, quadrature=quad)
+    ini.init(5)
+    y = ini.get_state()
+    dv, wq = inputs.v_weights(nv, quad)
+    assert abs((y[0, 0] * wq).sum() * dv - 1.0) < 1e-14 and abs((y[4, 0] * wq).sum() * dv - 0.9) < 1e-14
+    np.testing.assert_allclose(y, inputs.fast_conversion_state(32, nv, 5, quadrature=quad), rtol=1e-13, atol=1e-20)
+
+
+def test_quadrature_option_validation():
+    sim = R.RefSim(16, 4, 16.0, 0.1, 0, 0, 0, FD)
+    with pytest.raises(RuntimeError):
+        sim.set_option(R.OPT_QUADRATURE, 2)      # Simpson needs an odd number of points
+    with pytest.raises(RuntimeError):
+        sim.set_option(R.OPT_QUADRATURE, 3)
