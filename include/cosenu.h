@@ -60,8 +60,13 @@ enum {
                               default 2 */
   COSENU_OPT_STAGE_TIMING = 4, /* 1: bracket every stage launch with CUDA events on the handle's stream
                               (read with cosenu_stage_times); default 0 */
-  COSENU_OPT_VARIANT = 5   /* kernel shape: 0 = 8 compute warps x 2 rows (default), 1 = 16 compute warps x 1 row;
+  COSENU_OPT_VARIANT = 5,  /* kernel shape: 0 = 8 compute warps x 2 rows (default), 1 = 16 compute warps x 1 row;
                               same arithmetic per cell, different summation grouping of the moments only */
+  COSENU_OPT_QUADRATURE = 6 /* v-grid and rule of the v' integral of Eq. (3); must be set before init / set_state:
+                              0: nv bins represented by their centres v_j = -1 + (j + 1/2) 2/nv, Riemann sum (default)
+                              1: nv vertex-centred points v_j = -1 + 2 j/(nv-1), trapezoid rule (the FD variant of PAPER.md:82-86)
+                              2: the same points, Simpson's rule; needs nv odd, nv >= 3
+                              The same weights enter the v-sums of the diagnostics and the normalisation of cosenu_init. */
 };
 
 /* Diagnostics.  References are taken when a state is set. */

@@ -14,7 +14,7 @@ LIB_PATH = os.path.join(HERE, "libcosenu_b200.so")
 
 FD4_KO3, FV_WENO7 = 0, 1
 OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, 1, 2, 3, 4
-OPT_EPS_KO, OPT_WENO_EPS, OPT_ADVECT, OPT_RK_FORM, OPT_STAGE_TIMING, OPT_VARIANT = 0, 1, 2, 3, 4, 5
+OPT_EPS_KO, OPT_WENO_EPS, OPT_ADVECT, OPT_RK_FORM, OPT_STAGE_TIMING, OPT_VARIANT, OPT_QUADRATURE = 0, 1, 2, 3, 4, 5, 6
 
 # every symbol include/cosenu.h declares
 SYMBOLS = ["cosenu_create", "cosenu_workspace_bytes", "cosenu_attach", "cosenu_set_option", "cosenu_init",
@@ -83,7 +83,7 @@ class Cosenu:
     """One solver handle on the current CUDA device.  Method names mirror the C ABI."""
 
     def __init__(self, nz, nv, L, dt, omega, theta, mu, scheme, eps_ko=None, weno_eps=None, advect=True,
-                 rk_form=None, variant=0, use_torch_workspace=True, stream=None):
+                 rk_form=None, variant=0, quadrature=0, use_torch_workspace=True, stream=None):
         self._L = load()
         self.nz, self.nv = int(nz), int(nv)
         self.h = self._L.cosenu_create(nz, nv, L, dt, omega, theta, mu, scheme)
@@ -107,6 +107,8 @@ class Cosenu:
             self.set_option(OPT_RK_FORM, rk_form)
         if variant:
             self.set_option(OPT_VARIANT, variant)
+        if quadrature:
+            self.set_option(OPT_QUADRATURE, quadrature)
 
     def _chk(self, rc):
         if rc != 0:

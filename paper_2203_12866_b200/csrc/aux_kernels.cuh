@@ -6,6 +6,16 @@
 
 namespace cosenu_dev {
 
+// weight of beam j in the v' integral, in units of dv (int f dv ~ dv sum_j w_j f(v_j)):
+//   quad 0: bin centres + Riemann sum -> 1;  on the vertex-centred grid of the FD variant
+//   quad 1: trapezoid rule -> (1/2, 1, ..., 1, 1/2);  quad 2: Simpson's rule (nv odd) -> (1, 4, 2, ..., 4, 1)/3
+__host__ __device__ __forceinline__ double quad_weight(int j, int nv, int quad) {
+  if (quad == 0) return 1.0;
+  const bool end = (j == 0) || (j == nv - 1);
+  if (quad == 1) return end ? 0.5 : 1.0;
+  return end ? 1.0 / 3.0 : ((j & 1) ? 4.0 / 3.0 : 2.0 / 3.0);
+}
+
 // periodic ghost rows of one state buffer: rows -G..-1 <- nz-G..nz-1, rows nz..nz+G-1 <- 0..G-1
 __global__ void fill_ghosts_kernel(double* y, long long nz, int nvp, long long comp_stride, int g) {
   const long long n = (long long)8 * 2 * g * nvp;
@@ -22,16 +32,17 @@ __global__ void fill_ghosts_kernel(double* y, long long nz, int nvp, long long c
 // the 6 velocity moments per z of a state (S1; Riemann sum of PAPER.md:78): one warp per z row,
 // lanes stride over v, fixed shuffle tree => reproducible.  mom[6][nz], already times dv.
 __global__ void moments_kernel(const double* __restrict__ y, double* __restrict__ mom, long long nz, int nv, int nvp,
-                               long long comp_stride, int g, double dv) {
+                               long long comp_stride, int g, double dv, double voff, int quad) {
   const int warps = blockDim.x / 32, wid = threadIdx.x / 32, lane = threadIdx.x % 32;
   for (long long iz = blockIdx.x * (long long)warps + wid; iz < nz; iz += (long long)gridDim.x * warps) {
     double m[6] = {0, 0, 0, 0, 0, 0};
     const double* row = y + (iz + g) * nvp;
     for (int j = lane; j < nv; j += 32) {
-      const double v = __dadd_rn(-1.0, __dmul_rn((double)j + 0.5, dv));
-      const double dd = (row[j] - row[comp_stride + j]) - (row[4 * comp_stride + j] - row[5 * comp_stride + j]);
-      const double dr = row[2 * comp_stride + j] - row[6 * comp_stride + j];
-      const double di = row[3 * comp_stride + j] + row[7 * comp_stride + j];
+      const double v = __dadd_rn(-1.0, __dmul_rn((double)j + voff, dv));
+      const double wq = quad_weight(j, nv, quad);
+      const double dd = wq * ((row[j] - row[comp_stride + j]) - (row[4 * comp_stride + j] - row[5 * comp_stride + j]));
+      const double dr = wq * (row[2 * comp_stride + j] - row[6 * comp_stride + j]);
+      const double di = wq * (row[3 * comp_stride + j] + row[7 * comp_stride + j]);
       m[0] += dd; m[1] = fma(v, dd, m[1]);
       m[2] += dr; m[3] = fma(v, dr, m[3]);
       m[4] += di; m[5] = fma(v, di, m[5]);
@@ -78,13 +89,14 @@ constexpr int DIAG_NVAL = DIAG_NSUM + DIAG_NMAX;
 // per-block partial diagnostics over a z-slab: part[b][DIAG_NVAL]
 __global__ void diag_kernel(const double* __restrict__ y, const double* __restrict__ pref /*[2][nv]*/,
                             const double* __restrict__ p0ref /*[2][nv]*/, double* __restrict__ part, long long nz,
-                            int nv, int nvp, long long comp_stride, int g) {
+                            int nv, int nvp, long long comp_stride, int g, int quad) {
   const long long rows_per = (nz + gridDim.x - 1) / gridDim.x;
   const long long z0 = blockIdx.x * rows_per, z1 = min(nz, z0 + rows_per);
   double sm[DIAG_NSUM] = {0, 0, 0, 0, 0, 0, 0};
   double mx[DIAG_NMAX] = {0, 0, 0};
   for (int j = threadIdx.x; j < nv; j += blockDim.x) {
     const double pr[2] = {pref[j], pref[nv + j]}, p0[2] = {p0ref[j], p0ref[nv + j]};
+    const double wq = quad_weight(j, nv, quad);   // the v-sums of PAPER.md:229, Eq. (19), Eq. (23) use the rule of the v' integral
     for (long long iz = z0; iz < z1; ++iz) {
       const double* q = y + (iz + g) * nvp + j;
       double c[8];
@@ -93,17 +105,17 @@ __global__ void diag_kernel(const double* __restrict__ y, const double* __restri
 #pragma unroll
       for (int s = 0; s < 2; ++s) {
         const double ee = c[4 * s], xx = c[4 * s + 1], r = c[4 * s + 2], im = c[4 * s + 3];
-        sm[s] += ee;
+        sm[s] += wq * ee;
         const double P = plen(ee, xx, r, im);
         if (pr[s] > 0) mx[0] = fmax(mx[0], fabs(P / pr[s] - 1.0));   // Eq. (22)
-        if (s == 0) sm[2] += fabs(P - pr[0]);                        // numerator of Eq. (23)
+        if (s == 0) sm[2] += wq * fabs(P - pr[0]);                       // numerator of Eq. (23)
         mx[1] = fmax(mx[1], fabs(ee + xx - p0[s]));
         mx[2] = fmax(mx[2], sqrt(fma(r, r, im * im)));
       }
       // Eq. (19) in stored variables: P = (2 Re, -2 Im, ee - xx) of D = rho - rhobar^*
-      sm[3] += 2.0 * (c[2] - c[6]);
-      sm[4] += -2.0 * (c[3] + c[7]);
-      sm[5] += (c[0] - c[1]) - (c[4] - c[5]);
+      sm[3] += wq * (2.0 * (c[2] - c[6]));
+      sm[4] += wq * (-2.0 * (c[3] + c[7]));
+      sm[5] += wq * ((c[0] - c[1]) - (c[4] - c[5]));
     }
   }
   __shared__ double red[32][DIAG_NVAL];

@@ -40,7 +40,8 @@ struct cosenu {
   double L, dt, omega, theta, mu; int scheme;
   double eps_ko = 0.1, weno_eps = 1e-6;
   int advect = 1, rk_form = 2, stage_timing = 0;   // rk_form: 0 accumulator, 1 lean accumulator, 2 accumulator-free
-  double dz, dv;
+  int quad = 0;          // COSENU_OPT_QUADRATURE
+  double dz, dv, voff = 0.5;   // v_j = -1 + (j + voff) dv
   int device = 0;
   int variant = 0;       // kernel shape variant (COSENU_OPT_VARIANT)
   int num_sms = 148;
@@ -209,7 +210,7 @@ StageParams base_params(const cosenu* h) {
   p.mu = h->mu;
   p.A0 = -h->omega * std::cos(2.0 * h->theta);
   p.Br0 = 0.5 * h->omega * std::sin(2.0 * h->theta);
-  p.dv = h->dv;
+  p.dv = h->dv; p.voff = h->voff; p.quad = h->quad;
   const double sw = h->advect ? 1.0 : 0.0;
   p.cadv = sw * (-1.0 / (12.0 * h->dz));
   p.cko = sw * (-h->eps_ko / (16.0 * h->dz));
@@ -290,7 +291,7 @@ int one_step(cosenu* h) {
 
 int run_diag(cosenu* h, double sums[DIAG_NSUM], double maxs[DIAG_NMAX]) {
   diag_kernel<<<DIAG_BLOCKS, DIAG_THREADS, 0, h->stream>>>(h->U, h->d_pref, h->d_p0ref, h->d_diagpart, h->nz, h->nv,
-                                                           h->nvp, h->comp_stride, G);
+                                                           h->nvp, h->comp_stride, G, h->quad);
   CK(cudaGetLastError());
   h->launches++;
   std::vector<double> part((size_t)DIAG_BLOCKS * DIAG_NVAL);
@@ -312,7 +313,7 @@ int finish_upload(cosenu* h, double t) {
   fill_ghosts_kernel<<<64, 256, 0, h->stream>>>(h->U, h->nz, h->nvp, h->comp_stride, G);
   CK(cudaGetLastError());
   h->mcur = 0;
-  moments_kernel<<<592, 256, 0, h->stream>>>(h->U, h->M[0], h->nz, h->nv, h->nvp, h->comp_stride, G, h->dv);
+  moments_kernel<<<592, 256, 0, h->stream>>>(h->U, h->M[0], h->nz, h->nv, h->nvp, h->comp_stride, G, h->dv, h->voff, h->quad);
   CK(cudaGetLastError());
   diag_ref_kernel<<<REF_BLOCKS, 256, 0, h->stream>>>(h->U, h->d_refpart, h->nz, h->nv, h->nvp, h->comp_stride, G);
   CK(cudaGetLastError());
@@ -328,7 +329,7 @@ int finish_upload(cosenu* h, double t) {
       for (int m = 0; m < 4; ++m) a[m] += part[((size_t)b * 4 + m) * h->nv + j];
     pref[j] = (double)(a[0] / h->nz); p0ref[j] = (double)(a[1] / h->nz);
     pref[h->nv + j] = (double)(a[2] / h->nz); p0ref[h->nv + j] = (double)(a[3] / h->nz);
-    prsum += pref[j];
+    prsum += (long double)quad_weight(j, h->nv, h->quad) * pref[j];
   }
   h->pref_sum_nu = (double)(prsum * h->nz);
   CK(cudaMemcpyAsync(h->d_pref, pref.data(), sizeof(double) * pref.size(), cudaMemcpyHostToDevice, h->stream));
@@ -408,6 +409,13 @@ extern "C" int cosenu_set_option(cosenu_t* h, int key, double value) {
     case COSENU_OPT_ADVECT: h->advect = value != 0; return COSENU_OK;
     case COSENU_OPT_RK_FORM: if (value != 0 && value != 1 && value != 2) break; h->rk_form = (int)value; return COSENU_OK;
     case COSENU_OPT_VARIANT: if (value != 0 && value != 1) break; h->variant = (int)value; return COSENU_OK;
+    case COSENU_OPT_QUADRATURE:
+      if ((value != 0 && value != 1 && value != 2) || (value == 2 && (h->nv % 2 == 0 || h->nv < 3))) break;
+      if (h->have_state) return fail(h, COSENU_ESTATE, "cosenu_set_option: the quadrature must be chosen before init / set_state");
+      h->quad = (int)value;
+      h->voff = h->quad == 0 ? 0.5 : 0.0;
+      h->dv = h->quad == 0 ? 2.0 / (double)h->nv : 2.0 / (double)(h->nv - 1);
+      return COSENU_OK;
     case COSENU_OPT_STAGE_TIMING: {
       int rc = drain_events(h);
       if (rc) return rc;
@@ -444,10 +452,10 @@ extern "C" int cosenu_init(cosenu_t* h, uint64_t seed, double sigma_nu, double s
   std::vector<double> g(nv), gb(nv);
   double sg = 0, sgb = 0;
   for (int j = 0; j < nv; ++j) {
-    const double v = -1.0 + (j + 0.5) * h->dv;
+    const double v = -1.0 + ((double)j + h->voff) * h->dv, w = quad_weight(j, nv, h->quad);
     g[j] = std::exp(-(v - 1.0) * (v - 1.0) / (2.0 * sigma_nu * sigma_nu));
     gb[j] = std::exp(-(v - 1.0) * (v - 1.0) / (2.0 * sigma_nubar * sigma_nubar));
-    sg += g[j]; sgb += gb[j];
+    sg += w * g[j]; sgb += w * gb[j];
   }
   for (int j = 0; j < nv; ++j) { g[j] = g[j] / (sg * h->dv); gb[j] = alpha * (gb[j] / (sgb * h->dv)); }
   const double two_pi = 6.283185307179586476925286766559;

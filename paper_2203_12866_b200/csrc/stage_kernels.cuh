@@ -25,6 +25,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "aux_kernels.cuh"
 #include "weno7_math.h"
 
 namespace cosenu_dev {
@@ -49,7 +50,8 @@ struct StageParams {
   long long comp_stride;  // (nz + 2G) * nvp
   double cy, ca;          // y_out = base + cy k ; acc_out = acc_in + ca k
   double mu, A0, Br0;     // A0 = -omega cos 2theta, Br0 = (omega/2) sin 2theta
-  double dv;
+  double dv, voff;         // v_j = -1 + (j + voff) dv: voff = 1/2 bin centres, 0 vertex-centred
+  int quad;                // rule of the v' integral: 0 Riemann/midpoint, 1 trapezoid, 2 Simpson (aux_kernels.cuh: quad_weight)
   double cadv, cko;          // FD: -1/(12 dz), -eps_ko/(16 dz)   (times the advect switch)
   double ninv_dz, weno_eps;  // WENO: -1/dz (times the advect switch), epsilon of Eq. (14)
 };
@@ -350,8 +352,9 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
     const uint32_t Ta_in = Tu + KT::ACC_LOAD_ARR * SM::PTILE, Ta_out = Tu + SM::PTILE;
     const int j = ch * VC + lane;
     const bool active = j < p.nv;
-    // v_j = -1 + (j + 1/2) dv, formed without contraction
-    const double v = __dadd_rn(-1.0, __dmul_rn((double)j + 0.5, p.dv));
+    // v_j = -1 + (j + voff) dv, formed without contraction (vertex-centred variant PAPER.md:82-86)
+    const double v = __dadd_rn(-1.0, __dmul_rn((double)j + p.voff, p.dv));
+    const double wq = quad_weight(j, p.nv, p.quad);   // exactly 1 for the default Riemann sum
     mbar_wait(b_full_y + 8 * sy, (uint32_t)((n / NY) & 1));
 
     // ---- S2 (WENO7): right-interface fluxes of my rows, published for the neighbouring warp
@@ -510,7 +513,8 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
 
       // ---- S5: velocity moments of the produced state, D = rho - rhobar^*
       {
-        const double dd = (out[0] - out[1]) - (out[4] - out[5]), dr = out[2] - out[6], di = out[3] + out[7];
+        const double dd = wq * ((out[0] - out[1]) - (out[4] - out[5])), dr = wq * (out[2] - out[6]),
+                     di = wq * (out[3] + out[7]);
         msum[6 * s + 0] += dd;
         msum[6 * s + 1] = fma(v, dd, msum[6 * s + 1]);
         msum[6 * s + 2] += dr;

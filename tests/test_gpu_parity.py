@@ -36,7 +36,7 @@ def run_pair(B, R, args, st, nsteps, **opts):
     gm = g.get_moments()
     gd = g.diagnostics()
     g.close()
-    ropts = {k: v for k, v in opts.items() if k in ("eps_ko", "weno_eps", "advect")}
+    ropts = {k: v for k, v in opts.items() if k in ("eps_ko", "weno_eps", "advect", "quadrature")}
     r = R.RefSim(*args, **ropts)
     r.set_state(st)
     r.step(nsteps)
@@ -138,6 +138,41 @@ def test_eps_ko_option(B, R):
     assert np.max(np.abs(got - ref)) <= 1e-13
 
 
+@pytest.mark.parametrize("scheme", [FD, FV])
+@pytest.mark.parametrize("quad,nv", [(1, 16), (1, 45), (2, 17), (2, 129), (2, 3)])
+def test_quadrature_variants(B, R, scheme, quad, nv):
+    """Vertex-centred v-grid with the trapezoid / Simpson rule: state, moments and the weighted
+    diagnostics against the oracle, one step from a rough O(1) state and 20 steps of the fast-conversion recipe."""
+    nz = 200
+    st = inputs.random_state(nz, nv, seed=300 + nv)
+    args = (nz, nv, 0.7 * nz, 0.05, 0.8, 0.3, 1.3, scheme)
+    got, ref, gm, rm, gd, rd = run_pair(B, R, args, st, 1, quadrature=quad)
+    assert np.max(np.abs(got - ref)) <= 2e-14 * max(1.0, np.max(np.abs(ref)))
+    assert np.max(np.abs(gm - rm)) <= 1e-14 * max(1.0, np.max(np.abs(rm)))
+    st = inputs.fast_conversion_state(nz, nv, seed=41, pert_amp=1e-6, quadrature=quad)   # BASELINE recipe
+    args = (nz, nv, float(nz), 0.4, 1e-2, 0.01, 1.0, scheme)
+    got, ref, gm, rm, gd, rd = run_pair(B, R, args, st, 20, quadrature=quad)
+    assert np.max(np.abs(got - ref)) <= TOL20
+    assert np.max(np.abs(gm - rm)) <= TOL20
+    for k in ("psurv_nu", "psurv_nubar", "dP_max", "dP_avg", "trace_dev_max", "ex_abs_max"):
+        assert abs(gd[k] - rd[k]) <= 1e-11, k
+    assert np.max(np.abs(np.array(gd["M0"]) - np.array(rd["M0"]))) <= 1e-11
+    # discrete normalisation of Eq. (20) with the rule's own weights: M0_3(0) = (1 - alpha) L exactly (reading A14)
+    assert abs(gd["M0"][2] - gd["dM0"][2] - 0.1 * nz) <= 1e-10
+
+
+def test_quadrature_option_rules(B):
+    g = B.Cosenu(64, 16, 64.0, 0.1, 0, 0, 1.0, FD)
+    with pytest.raises(B.CosenuError):
+        g.set_option(B.OPT_QUADRATURE, 2)           # Simpson needs an odd number of points
+    g.set_option(B.OPT_QUADRATURE, 1)
+    g.init(3)
+    with pytest.raises(B.CosenuError) as e:
+        g.set_option(B.OPT_QUADRATURE, 0)           # the grid is fixed once a state exists
+    assert e.value.code == B.ESTATE
+    g.close()
+
+
 def test_init_matches_oracle_init(B, R):
     """cosenu_init (library-side generator) gives bit-identical states to the oracle's and the input module's."""
     for kind in (0, 1, 2):
@@ -150,6 +185,16 @@ def test_init_matches_oracle_init(B, R):
         b = r.get_state()
         r.close()
         assert np.array_equal(a, b), kind
+    for quad, nv in ((1, 20), (2, 21)):
+        g = B.Cosenu(512, nv, 512.0, 0.4, 0.0, 0.0, 1.0, FD, quadrature=quad)
+        g.init(12866)
+        a = g.get_state()
+        g.close()
+        r = R.RefSim(512, nv, 512.0, 0.4, 0.0, 0.0, 1.0, FD, quadrature=quad)
+        r.init(12866)
+        b = r.get_state()
+        r.close()
+        assert np.array_equal(a, b), quad
     # the numpy recipe differs from the C generators only by libm-vs-numpy rounding of cos/sin/exp
     np.testing.assert_allclose(_init_state(B, 512, 20, 12866), inputs.fast_conversion_state(512, 20, 12866),
                                rtol=1e-14, atol=1e-21)
