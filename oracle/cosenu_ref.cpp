@@ -27,6 +27,7 @@ struct cosenu_ref {
   double eps_ko = 0.1;      // PAPER.md:164 "KO3 with eps_KO = 0.1"
   double weno_eps = 1e-6;   // PAPER.md:145 "typical value ~1e-6"
   int advect = 1; int threads = 0; int quad = 0;
+  int ko_r = 2;             // order r of the Kreiss-Oliger operator, Eq. (5): "we have used r = 2 for most"
   double dz, dv;
   std::vector<double> v;    // beam velocities: bin centres or vertex-centred points
   std::vector<double> wq;   // quadrature weights in units of dv: int f dv ~ dv * sum_j wq_j f(v_j)
@@ -152,7 +153,14 @@ static void rhs(const cosenu_ref* h, const double* y, double* k) {
           const double dudz = (um2 - 8.0 * um1 + 8.0 * up1 - up2) / (12.0 * h->dz);
           // Kreiss-Oliger r=2, Eq. (5) with the dissipative sign (reading A4):
           //   Q u = -(eps/16 dz) (u_{i-2} - 4u_{i-1} + 6u_i - 4u_{i+1} + u_{i+2})
-          const double ko = (h->eps_ko / (16.0 * h->dz)) * (um2 - 4.0 * um1 + 6.0 * u0 - 4.0 * up1 + up2);
+          double ko = (h->eps_ko / (16.0 * h->dz)) * (um2 - 4.0 * um1 + 6.0 * u0 - 4.0 * up1 + up2);
+          if (h->ko_r == 3) {
+            // Eq. (5) with r = 3: eps h^5 (D+ D-)^3 / 2^6 = (eps / 64 dz) (u_{i-3} - 6u_{i-2} + 15u_{i-1} - 20u_i + 15u_{i+1}
+            // - 6u_{i+2} + u_{i+3}); dissipative sign (reading A4): its Fourier symbol is -(eps/dz) sin^6(k dz/2), so it is
+            // ADDED here where the r = 2 term is subtracted ((D+ D-)^r alternates in sign with r)
+            const double um3 = y[idx(h, c, wrap(i - 3, nz), j)], up3 = y[idx(h, c, wrap(i + 3, nz), j)];
+            ko = -(h->eps_ko / (64.0 * h->dz)) * (um3 - 6.0 * um2 + 15.0 * um1 - 20.0 * u0 + 15.0 * up1 - 6.0 * up2 + up3);
+          }
           k[idx(h, c, i, j)] = -h->v[j] * dudz - ko;
         }
     }
@@ -290,6 +298,7 @@ extern "C" int cosenu_ref_set_option(cosenu_ref_t* h, int key, double value) {
     case COSENU_REF_OPT_WENO_EPS: if (!(value > 0)) break; h->weno_eps = value; return COSENU_REF_OK;
     case COSENU_REF_OPT_ADVECT: h->advect = value != 0; return COSENU_REF_OK;
     case COSENU_REF_OPT_THREADS: if (value < 0) break; h->threads = (int)value; return COSENU_REF_OK;
+    case COSENU_REF_OPT_KO_ORDER: if (value != 2 && value != 3) break; h->ko_r = (int)value; return COSENU_REF_OK;
     case COSENU_REF_OPT_QUADRATURE:
       if ((value != 0 && value != 1 && value != 2) || h->have_state || (value == 2 && (h->nv % 2 == 0 || h->nv < 3))) break;
       h->quad = (int)value; build_vgrid(h); return COSENU_REF_OK;

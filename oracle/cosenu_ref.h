@@ -35,6 +35,7 @@ enum { COSENU_REF_OPT_EPS_KO = 0,    /* KO strength, default 0.1 
        COSENU_REF_OPT_WENO_EPS = 1,  /* epsilon of Eq. (14), default 1e-6 */
        COSENU_REF_OPT_ADVECT = 2,    /* test hook: 0 switches the advection term off */
        COSENU_REF_OPT_THREADS = 3,   /* OpenMP threads over z (0 = all) */
+       COSENU_REF_OPT_KO_ORDER = 5,  /* r of Eq. (5): 2 (default) or 3 (7-point operator, halo 3) */
        COSENU_REF_OPT_QUADRATURE = 4 }; /* v-grid and rule of the v' integral (set before init / set_state):
                                         0 bin centres + Riemann sum (default);
                                         1 vertex-centred points v_j = -1 + 2j/(nv-1) + trapezoid rule;

@@ -7,7 +7,7 @@ import numpy as np
 from . import build_oracle
 
 FD4_KO3, FV_WENO7 = 0, 1
-OPT_EPS_KO, OPT_WENO_EPS, OPT_ADVECT, OPT_THREADS, OPT_QUADRATURE = 0, 1, 2, 3, 4
+OPT_EPS_KO, OPT_WENO_EPS, OPT_ADVECT, OPT_THREADS, OPT_QUADRATURE, OPT_KO_ORDER = 0, 1, 2, 3, 4, 5
 
 
 class Diag(C.Structure):
@@ -68,7 +68,7 @@ class RefSim:
     """Thin wrapper over the cosenu_ref_* C ABI (same call names as the product binding)."""
 
     def __init__(self, nz, nv, L, dt, omega, theta, mu, scheme, eps_ko=None, weno_eps=None,
-                 advect=True, threads=0, quadrature=0):
+                 advect=True, threads=0, quadrature=0, ko_order=2):
         self._L = lib()
         self.nz, self.nv = int(nz), int(nv)
         self.h = self._L.cosenu_ref_create(nz, nv, L, dt, omega, theta, mu, scheme)
@@ -84,6 +84,8 @@ class RefSim:
             self.set_option(OPT_THREADS, threads)
         if quadrature:
             self.set_option(OPT_QUADRATURE, quadrature)
+        if ko_order != 2:
+            self.set_option(OPT_KO_ORDER, ko_order)
 
     def _chk(self, rc):
         if rc != 0:

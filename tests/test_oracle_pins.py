@@ -64,10 +64,12 @@ def linear_closed_form(st0, nsteps, dt, omega, theta, lam_adv):
     return out
 
 
-def fd_ko_symbol(nz, nv, dz, eps_ko):
+def fd_ko_symbol(nz, nv, dz, eps_ko, r=2):
+    """Fourier symbol of FD4 + Kreiss-Oliger of order r: Eq. (5) with the dissipative sign is
+    -(eps/dz) sin^{2r}(k dz/2), since D+ D- -> -(4/dz^2) sin^2(k dz/2)."""
     th = 2 * np.pi * np.fft.fftfreq(nz)[:, None]  # k dz
     v = inputs.v_grid(nv)[None, :]
-    return -1j * v * (8 * np.sin(th) - np.sin(2 * th)) / (6 * dz) - (eps_ko / dz) * np.sin(th / 2) ** 4
+    return -1j * v * (8 * np.sin(th) - np.sin(2 * th)) / (6 * dz) - (eps_ko / dz) * np.sin(th / 2) ** (2 * r)
 
 
 def weno_linear_symbol(nz, nv, dz):
@@ -301,6 +303,46 @@ def test_P4_ko_damps_nyquist_mode():
     assert np.allclose(k, -eps * st[0], atol=1e-15)
     sim.set_state(st); sim.step(500)
     assert np.allclose(sim.get_state()[0], st[0] * np.exp(-eps * 5.0), rtol=1e-9)
+
+
+# ----------------------------------------------------------------------------- KO with r = 3 (Eq. 5, general r)
+def test_ko_r3_closed_form_nyquist_and_order():
+    """Eq. (5) with r = 3 ("general form of the 2r-order Kreiss-Oliger dissipation"): a 7-point
+    operator with symbol -(eps/dz) sin^6(k dz/2).  Pins: the DFT closed form on white noise, the Nyquist mode
+    (same decay rate as r = 2 because sin(pi/2) = 1), exact zero on quintic polynomials' 6th difference, and the
+    convergence order: the r = 3 term is O(dz^5), so FD4 keeps its 4th order (r = 2 lowers it to 3)."""
+    nz, nv, dt, nsteps = 96, 6, 0.4, 100
+    st = inputs.random_state(nz, nv, 81)
+    sim = R.RefSim(nz, nv, float(nz), dt, 0.7, 0.3, 0.0, FD, eps_ko=0.25, ko_order=3)
+    sim.set_state(st); sim.step(nsteps)
+    want = linear_closed_form(st, nsteps, dt, 0.7, 0.3, fd_ko_symbol(nz, nv, 1.0, 0.25, r=3))
+    assert np.abs(sim.get_state() - want).max() < 5e-14
+    # Nyquist mode: k = Q u = -(eps/dz) u
+    nz, nv, eps = 32, 2, 0.1
+    sim = R.RefSim(nz, nv, float(nz), 0.01, 0.0, 0.0, 0.0, FD, eps_ko=eps, ko_order=3)
+    u = np.zeros((8, nz, nv)); u[0] = ((-1.0) ** np.arange(nz))[:, None]
+    assert np.allclose(sim.rhs(u)[0], -eps * u[0], atol=1e-15)
+    # one Fourier mode k: the r = 3 and r = 2 operators differ by the factor sin^2(k dz/2)
+    kk = 5
+    u[0] = np.cos(2 * np.pi * kk * np.arange(nz) / nz)[:, None]
+    sim0 = R.RefSim(nz, nv, float(nz), 0.01, 0.0, 0.0, 0.0, FD, eps_ko=0.0)
+    sim2 = R.RefSim(nz, nv, float(nz), 0.01, 0.0, 0.0, 0.0, FD, eps_ko=eps)
+    q3 = sim.rhs(u)[0] - sim0.rhs(u)[0]
+    q2 = sim2.rhs(u)[0] - sim0.rhs(u)[0]
+    assert np.allclose(q3, q2 * np.sin(np.pi * kk / nz) ** 2, atol=1e-15)
+    # order of convergence with the dissipation on
+    e = []
+    for n in (32, 64):
+        nvv, L, T = 2, 2 * np.pi, 2.0
+        dz = L / n
+        ns = int(np.ceil(T / (0.02 * dz))); dtt = T / ns
+        s3 = R.RefSim(n, nvv, L, dtt, 0.0, 0.0, 0.0, FD, eps_ko=0.1, ko_order=3)
+        zl = np.arange(n) * dz
+        st = np.zeros((8, n, nvv)); st[0] = np.sin(zl)[:, None]
+        s3.set_state(st); s3.step(ns)
+        v = inputs.v_grid(nvv)
+        e.append(max(np.sqrt(np.mean((s3.get_state()[0][:, j] - np.sin(zl - v[j] * T)) ** 2)) for j in range(nvv)))
+    assert abs(np.log2(e[0] / e[1]) - 4.0) < 0.3
 
 
 # ----------------------------------------------------------------------------- P6: WENO linear limit
