@@ -10,9 +10,12 @@ A "step" is one classical RK4 step (4 fused stage launches) of the whole (z,v) g
 (paper_2203_12866_b200/inputs.py); the state (>= 2 GB per copy) is far larger than L2, so no L2 flush
 is needed between steps.
 
-N > 1 (torchrun): every rank owns an independent replica of the workload on its own GPU (weak scaling,
-no data-path collective: the z-slab halo exchange is a NEXT item); barrier +
-max-over-ranks timing; value = total cells of all ranks / that time.
+N > 1 (torchrun): by default every rank owns an independent replica of the workload on its own GPU (weak
+scaling, no data-path collective; the north star is a one-GPU path).  `--decomp slab` runs ONE periodic grid
+of N x nz rows cut into z-slabs, one per rank: the halo exchange is fused into the stage kernels (peer stores
+over NVLink + arrival counters); still weak scaling (nz rows per GPU).  Barrier +
+max-over-ranks timing; value = total cells of all ranks / that time.  With N = 1, `--decomp slab` runs the
+slab code path on a slab linked to itself.
 
 --impl reference: the CPU oracle (oracle/, as it stands) timed on the host cores on a bounded sample of
 the same workload (rank 0 only).
@@ -187,11 +190,25 @@ def run_ours(args):
     # ---- synthetic seeded input, built on the host in pinned memory (the e2e leg copies from it)
     host = torch.empty((8, nz, nv), dtype=torch.float64, pin_memory=True)
     hnp = host.numpy()
-    hnp[...] = inputs.fast_conversion_state(nz, nv, c["seed"] + rank) if c["kind"] == "fast" else \
-        inputs.vacuum_check_state(nz, nv, c["seed"] + rank)
-    sim = B.Cosenu(nz, nv, c["L"], c["dt"], c["omega"], c["theta"], c["mu"], c["scheme"], rk_form=args.rk_form,
-                   variant=args.variant)
-    sim.set_state(host)
+    if args.decomp != "slab":
+        hnp[...] = inputs.fast_conversion_state(nz, nv, c["seed"] + rank) if c["kind"] == "fast" else \
+            inputs.vacuum_check_state(nz, nv, c["seed"] + rank)
+    if args.decomp == "slab":
+        # one periodic grid of world * nz rows, this rank's slab of nz rows; the library builds the slab's rows of the
+        # seeded global state (cosenu_init enters the splitmix64 stream at z_begin)
+        if c["kind"] != "fast":
+            raise SystemExit("bench.py --decomp slab: fast-conversion workloads only")
+        from paper_2203_12866_b200 import slab as S
+        sim = S.CosenuSlab(world * nz, nv, world * c["L"], c["dt"], c["omega"], c["theta"], c["mu"], c["scheme"],
+                           rk_form=args.rk_form, variant=args.variant)
+        sim.init(c["seed"])
+        sim.get_state(host)
+        api = sim.sim
+    else:
+        sim = B.Cosenu(nz, nv, c["L"], c["dt"], c["omega"], c["theta"], c["mu"], c["scheme"], rk_form=args.rk_form,
+                       variant=args.variant)
+        sim.set_state(host)
+        api = sim
     d0 = sim.diagnostics()
 
     def barrier():
@@ -206,7 +223,7 @@ def run_ours(args):
     if rank == 0:
         sampler.start()
         time.sleep(0.15)
-    sim.set_option(B.OPT_STAGE_TIMING, 1)       # CUDA events around every stage launch, on the launching stream
+    api.set_option(B.OPT_STAGE_TIMING, 1)       # CUDA events around every stage launch, on the launching stream
     l0 = sim.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
@@ -216,11 +233,23 @@ def run_ours(args):
     barrier()
     ms = e0.elapsed_time(e1)
     launches = sim.launch_count() - l0
-    stage_ms, nst = sim.stage_times()
-    sim.set_option(B.OPT_STAGE_TIMING, 0)
+    stage_ms, nst = api.stage_times()
+    api.set_option(B.OPT_STAGE_TIMING, 0)
     clocks = sampler.stop() if rank == 0 else None
     ms = max_over_ranks(ms)
     value = whole_job_value(cells, args.steps, world, ms)
+
+    # ---- the same K steps without the per-stage events: cosenu_step replays its CUDA graph (8 steps per launch) when
+    # it may (single domain).  Matters on the small, launch-bound grids only; reported beside `value`.
+    barrier()
+    e0.record()
+    sim.step(args.steps)
+    e1.record()
+    barrier()
+    ms_graph = max_over_ranks(e0.elapsed_time(e1))
+    graph_replay = {"value": whole_job_value(cells, args.steps, world, ms_graph), "unit": UNIT,
+                    "ms_per_step": ms_graph / args.steps,
+                    "what": "same K steps, no per-stage events; CUDA-graph replay when steps >= 16 and single domain"}
 
     # ---- invariants at the bench size (properties that hold at any size)
     d1 = sim.diagnostics()
@@ -277,9 +306,11 @@ def run_ours(args):
            "config": {"workload": c["name"], "scheme": "FV_WENO7" if c["scheme"] else "FD4_KO3", "nz": nz, "nv": nv,
                       "dt": c["dt"], "omega": c["omega"], "theta": c["theta"], "mu": c["mu"],
                       "state_bytes_per_copy": state_bytes, "l2": "inputs larger than L2 (no flush needed)",
-                      "parallelism": "replicas x%d" % world, "rk_form": args.rk_form, "variant": args.variant},
+                      "parallelism": ("z-slabs x%d of one grid of %d rows (halo exchange fused into the stage kernels)"
+                                      % (world, world * nz)) if args.decomp == "slab" else "replicas x%d" % world,
+                      "rk_form": args.rk_form, "variant": args.variant},
            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
-           "checks": checks}
+           "graph_replay": graph_replay, "checks": checks}
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
@@ -296,6 +327,7 @@ def main():
     ap.add_argument("--rk-form", type=int, default=2, choices=[0, 1, 2])
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"])
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3

@@ -62,6 +62,13 @@ enum {
                               (read with cosenu_stage_times); default 0 */
   COSENU_OPT_VARIANT = 5,  /* kernel shape: 0 = 8 compute warps x 2 rows (default), 1 = 16 compute warps x 1 row;
                               same arithmetic per cell, different summation grouping of the moments only */
+  COSENU_OPT_GRAPH = 8,    /* 1 (default): cosenu_step(n >= 16) replays a CUDA graph of 8 RK4 steps (32 kernel nodes) captured from the
+                              handle's own launches, which removes the per-launch host cost on the small, launch-bound grids;
+                              0: always launch kernel by kernel.  Not used on slab handles (their launch parameters change every
+                              stage) nor while COSENU_OPT_STAGE_TIMING is on. */
+  COSENU_OPT_KO_ORDER = 7, /* r of the Kreiss-Oliger operator of Eq. (5): 2 (default; "r = 2 for most numerical
+                              experiments"; 5-point, halo 2) or 3 (7-point (eps/64dz) delta^6, halo 3).  FD scheme only;
+                              the handle's stream is idle when this is changed. */
   COSENU_OPT_QUADRATURE = 6 /* v-grid and rule of the v' integral of Eq. (3); must be set before init / set_state:
                               0: nv bins represented by their centres v_j = -1 + (j + 1/2) 2/nv, Riemann sum (default)
                               1: nv vertex-centred points v_j = -1 + 2 j/(nv-1), trapezoid rule (the FD variant of PAPER.md:82-86)
@@ -93,7 +100,8 @@ cosenu_t* cosenu_create(int64_t nz, int32_t nv, double L, double dt,
 size_t cosenu_workspace_bytes(const cosenu_t* h);
 
 /* Optional: use caller-owned device memory (>= cosenu_workspace_bytes, 256-byte aligned) and a
- * caller-owned cudaStream_t (NULL = legacy default stream).  Must be called before init/set_state;
+ * caller-owned cudaStream_t (NULL: the library creates a blocking stream of its own, which orders with the legacy default
+ * stream like default-stream work does).  Must be called before init/set_state;
  * if it never is, the library allocates its own workspace with cudaMalloc on first use. */
 int cosenu_attach(cosenu_t* h, void* dev_workspace, size_t bytes, void* cuda_stream);
 
@@ -111,7 +119,8 @@ int cosenu_init(cosenu_t* h, uint64_t seed, double sigma_nu, double sigma_nubar,
 /* Upload an arbitrary state (canonical host layout) and set the time. */
 int cosenu_set_state(cosenu_t* h, const double* host_state, double t);
 
-/* Advance n >= 0 RK4 steps: 4 n kernel launches enqueued on the stream, returns without waiting. */
+/* Advance n >= 0 RK4 steps: 4 n kernel launches (kernel by kernel, or as CUDA-graph replays, COSENU_OPT_GRAPH) enqueued on
+ * the stream; returns without waiting. */
 int cosenu_step(cosenu_t* h, int64_t n);
 
 /* Wait for the stream and copy the state to host_out (canonical host layout, 8*nz*nv doubles). */
@@ -138,6 +147,79 @@ int cosenu_stage_times(cosenu_t* h, double* ms_sum, int64_t* launches_per_stage)
 
 void cosenu_destroy(cosenu_t* h);
 const char* cosenu_last_error(const cosenu_t* h);
+
+/* ===================================================================================================
+ * z-slab decomposition over several GPUs (the paper's "future work").
+ *
+ * The periodic z-grid of nz_global cells is cut into contiguous slabs, one handle (one GPU, one process)
+ * per slab.  Everything a cell needs from other cells is (i) all beams v at its own z (the velocity
+ * moments of Eq. 3 are local in z, so a slab needs NO reduction collective) and (ii) the stencil halo in z
+ * (2 rows for FD4+KO3, 4 for WENO7).  The halo exchange is fused into the stage kernels: the CTA that
+ * produces the first / last 4 rows of a stage output also stores them into the neighbouring slab's ghost
+ * rows through peer memory (NVLink), then bumps an arrival counter in the neighbour's memory
+ * (release, system scope); the neighbour's next stage launch waits on that counter (acquire) only before it
+ * loads a tile that touches ghost rows.  Edge tiles are walked first, so the wait is normally over before
+ * it starts.  No host synchronisation and no extra launch per stage.
+ *
+ * Call order on every rank:  create_slab -> [attach(NULL, 0, stream)] -> set options -> slab_export ->
+ * (exchange the cosenu_slab_peer_t blobs) -> slab_link -> init / set_state (the LOCAL rows) ->
+ * slab_push_ghosts -> (barrier over all ranks) -> slab_ref_sums -> (sum over ranks) -> slab_set_ref_sums ->
+ * slab_diag_sums -> (reduce) -> slab_diag_finish(set_reference = 1) -> step ... ; all ranks must advance
+ * by the same number of steps.  cosenu_diagnostics is not available on a slab handle (ESTATE): use
+ * slab_diag_sums + reduce + slab_diag_finish.
+ * =================================================================================================== */
+
+/* What a neighbour needs to reach this slab's ghost rows and counters.  Plain data, safe to send between
+ * processes as bytes. */
+typedef struct {
+  unsigned char ipc_handle[64]; /* cudaIpcMemHandle_t of the allocation that holds the workspace */
+  uint64_t ipc_offset;          /* byte offset of the workspace inside that allocation */
+  uint64_t dev_base;            /* device address of the workspace in the exporting process */
+  int64_t  pid;                 /* exporting process (same pid => linked through dev_base, no IPC) */
+  int32_t  device;              /* CUDA device ordinal in the exporting process */
+  int32_t  nvp;                 /* row pitch in doubles */
+  int64_t  nz_local;            /* rows of the slab */
+  int64_t  comp_stride;         /* doubles between two components of a state buffer */
+  uint64_t off_buf[4];          /* byte offsets of the four state buffers inside the workspace */
+  uint64_t off_ctr;             /* byte offset of the two arrival counters (low ghosts, high ghosts) */
+} cosenu_slab_peer_t;
+
+/* A slab that owns rows [z_begin, z_begin + nz_local) of a periodic grid of nz_global cells; dz = L/nz_global.
+ * nz_local >= 16.  (nz_local == nz_global, linked to itself, is the single-domain solver again.) */
+cosenu_t* cosenu_create_slab(int64_t nz_global, int64_t z_begin, int64_t nz_local, int32_t nv, double L, double dt,
+                             double omega, double theta, double mu, int scheme);
+
+/* Allocate the workspace if needed (a slab that is reached over IPC should own its workspace: call
+ * cosenu_attach with dev_workspace = NULL to pass only the stream) and describe it. */
+int cosenu_slab_export(cosenu_t* h, cosenu_slab_peer_t* out);
+
+/* Connect to the slab below (lo: holds rows just before z_begin, periodically) and above (hi).  Peers of the same
+ * process are used through their device addresses; others are mapped with cudaIpcOpenMemHandle. */
+int cosenu_slab_link(cosenu_t* h, const cosenu_slab_peer_t* lo, const cosenu_slab_peer_t* hi);
+
+/* After init / set_state: store my edge rows into the neighbours' ghost rows (enqueued on the stream) and wait
+ * for the stream.  The caller then synchronises all ranks before the first step. */
+int cosenu_slab_push_ghosts(cosenu_t* h);
+
+/* Diagnostics of a decomposed run are sums / maxima over slabs; the caller supplies the reduction.
+ *  slab_ref_sums:     out[4][nv] = sum over my rows of |P_nu|, P0_nu, |P_nubar|, P0_nubar per beam
+ *  slab_set_ref_sums: the same array summed over all slabs -> the per-beam references of Eq. (22, 23)
+ *  slab_diag_sums:    out[10] = 7 sums then 3 maxima over my cells (opaque to the caller: reduce [0..6] by
+ *                     sum and [7..9] by max over the slabs)
+ *  slab_diag_finish:  global[10] -> *out; set_reference != 0 also stores the t = 0 references (survival
+ *                     probability denominators, M0(0)) */
+int cosenu_slab_ref_sums(cosenu_t* h, double* out);
+int cosenu_slab_set_ref_sums(cosenu_t* h, const double* global_sums);
+int cosenu_slab_diag_sums(cosenu_t* h, double* out10);
+int cosenu_slab_diag_finish(cosenu_t* h, const double* global10, int set_reference, cosenu_diag_t* out);
+
+/* Several slabs driven by ONE process on ONE stream (e.g. two slabs on one GPU in the tests): advances all of
+ * them n steps, stage by stage (every slab's stage k is enqueued before any slab's stage k+1, so no kernel ever
+ * waits for a kernel that is queued behind it). */
+int cosenu_slab_step_group(cosenu_t** hs, int32_t count, int64_t n);
+
+/* 1 if a halo wait of this handle ever timed out (a neighbour did not arrive within ~4 s); synchronises. */
+int cosenu_slab_wait_failed(cosenu_t* h, int32_t* failed);
 
 #ifdef __cplusplus
 }

@@ -14,12 +14,15 @@ LIB_PATH = os.path.join(HERE, "libcosenu_b200.so")
 
 FD4_KO3, FV_WENO7 = 0, 1
 OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, 1, 2, 3, 4
-OPT_EPS_KO, OPT_WENO_EPS, OPT_ADVECT, OPT_RK_FORM, OPT_STAGE_TIMING, OPT_VARIANT, OPT_QUADRATURE = 0, 1, 2, 3, 4, 5, 6
+OPT_EPS_KO, OPT_WENO_EPS, OPT_ADVECT, OPT_RK_FORM, OPT_STAGE_TIMING, OPT_VARIANT, OPT_QUADRATURE, OPT_KO_ORDER, OPT_GRAPH = 0, 1, 2, 3, 4, 5, 6, 7, 8
 
 # every symbol include/cosenu.h declares
 SYMBOLS = ["cosenu_create", "cosenu_workspace_bytes", "cosenu_attach", "cosenu_set_option", "cosenu_init",
            "cosenu_set_state", "cosenu_step", "cosenu_get_state", "cosenu_get_moments", "cosenu_diagnostics",
-           "cosenu_sync", "cosenu_launch_count", "cosenu_stage_times", "cosenu_destroy", "cosenu_last_error"]
+           "cosenu_sync", "cosenu_launch_count", "cosenu_stage_times", "cosenu_destroy", "cosenu_last_error",
+           "cosenu_create_slab", "cosenu_slab_export", "cosenu_slab_link", "cosenu_slab_push_ghosts",
+           "cosenu_slab_ref_sums", "cosenu_slab_set_ref_sums", "cosenu_slab_diag_sums", "cosenu_slab_diag_finish",
+           "cosenu_slab_step_group", "cosenu_slab_wait_failed"]
 
 
 class Diag(C.Structure):
@@ -34,6 +37,13 @@ class Diag(C.Structure):
                 "psurv_nubar": self.psurv_nubar, "dP_max": self.dP_max, "dP_avg": self.dP_avg,
                 "M0": list(self.M0), "dM0": list(self.dM0),
                 "trace_dev_max": self.trace_dev_max, "ex_abs_max": self.ex_abs_max}
+
+
+class SlabPeer(C.Structure):
+    """cosenu_slab_peer_t: what a neighbouring slab needs to reach this slab's ghost rows (plain bytes)."""
+    _fields_ = [("ipc_handle", C.c_ubyte * 64), ("ipc_offset", C.c_uint64), ("dev_base", C.c_uint64),
+                ("pid", C.c_int64), ("device", C.c_int32), ("nvp", C.c_int32), ("nz_local", C.c_int64),
+                ("comp_stride", C.c_int64), ("off_buf", C.c_uint64 * 4), ("off_ctr", C.c_uint64)]
 
 
 _lib = None
@@ -69,6 +79,17 @@ def load():
     L.cosenu_destroy.argtypes = [C.c_void_p]
     L.cosenu_last_error.restype = C.c_char_p
     L.cosenu_last_error.argtypes = [C.c_void_p]
+    L.cosenu_create_slab.restype = C.c_void_p
+    L.cosenu_create_slab.argtypes = [C.c_int64, C.c_int64, C.c_int64, C.c_int32] + [C.c_double] * 5 + [C.c_int]
+    L.cosenu_slab_export.argtypes = [C.c_void_p, C.POINTER(SlabPeer)]
+    L.cosenu_slab_link.argtypes = [C.c_void_p, C.POINTER(SlabPeer), C.POINTER(SlabPeer)]
+    L.cosenu_slab_push_ghosts.argtypes = [C.c_void_p]
+    L.cosenu_slab_ref_sums.argtypes = [C.c_void_p, dp]
+    L.cosenu_slab_set_ref_sums.argtypes = [C.c_void_p, dp]
+    L.cosenu_slab_diag_sums.argtypes = [C.c_void_p, dp]
+    L.cosenu_slab_diag_finish.argtypes = [C.c_void_p, dp, C.c_int, C.POINTER(Diag)]
+    L.cosenu_slab_step_group.argtypes = [C.POINTER(C.c_void_p), C.c_int32, C.c_int64]
+    L.cosenu_slab_wait_failed.argtypes = [C.c_void_p, C.POINTER(C.c_int32)]
     _lib = L
     return L
 
@@ -83,13 +104,20 @@ class Cosenu:
     """One solver handle on the current CUDA device.  Method names mirror the C ABI."""
 
     def __init__(self, nz, nv, L, dt, omega, theta, mu, scheme, eps_ko=None, weno_eps=None, advect=True,
-                 rk_form=None, variant=0, quadrature=0, use_torch_workspace=True, stream=None):
+                 rk_form=None, variant=0, quadrature=0, ko_order=2, graph=None, use_torch_workspace=True, stream=None, slab=None):
+        """slab = (nz_global, z_begin): this handle owns rows [z_begin, z_begin + nz) of a periodic grid of nz_global
+        cells (cosenu_create_slab; see slab.py for the drivers)."""
         self._L = load()
         self.nz, self.nv = int(nz), int(nv)
-        self.h = self._L.cosenu_create(nz, nv, L, dt, omega, theta, mu, scheme)
+        if slab is None:
+            self.h = self._L.cosenu_create(nz, nv, L, dt, omega, theta, mu, scheme)
+        else:
+            self.h = self._L.cosenu_create_slab(int(slab[0]), int(slab[1]), nz, nv, L, dt, omega, theta, mu, scheme)
         if not self.h:
             raise CosenuError(EINVAL, self._L.cosenu_last_error(None).decode())
         self._ws = None
+        if slab is not None and not use_torch_workspace and stream is not None:
+            self._chk(self._L.cosenu_attach(self.h, None, 0, stream.cuda_stream))   # library-owned memory, caller's stream
         if use_torch_workspace:
             import torch
             nbytes = self._L.cosenu_workspace_bytes(self.h)
@@ -109,6 +137,10 @@ class Cosenu:
             self.set_option(OPT_VARIANT, variant)
         if quadrature:
             self.set_option(OPT_QUADRATURE, quadrature)
+        if ko_order != 2:
+            self.set_option(OPT_KO_ORDER, ko_order)
+        if graph is not None:
+            self.set_option(OPT_GRAPH, 1 if graph else 0)
 
     def _chk(self, rc):
         if rc != 0:

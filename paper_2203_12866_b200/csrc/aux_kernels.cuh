@@ -29,6 +29,21 @@ __global__ void fill_ghosts_kernel(double* y, long long nz, int nvp, long long c
   }
 }
 
+// z-slab: copies of my first / last g rows of one state buffer into the neighbouring slabs' ghost rows (same
+// destinations as the stage kernels use, see StageParams::ghost_*_dst); used once after an upload
+__global__ void push_ghosts_kernel(const double* __restrict__ y, long long nz, int nvp, long long comp_stride, int g,
+                                   double* dst_lo, long long stride_lo, double* dst_hi, long long stride_hi) {
+  const long long n = (long long)8 * 2 * g * nvp;
+  for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < n; q += (long long)gridDim.x * blockDim.x) {
+    const int j = (int)(q % nvp);
+    const int r = (int)((q / nvp) % (2 * g));
+    const int c = (int)(q / ((long long)nvp * 2 * g));
+    const double* src = y + c * comp_stride;
+    if (r < g) dst_lo[c * stride_lo + (long long)r * nvp + j] = src[(long long)(g + r) * nvp + j];              // my row r
+    else dst_hi[c * stride_hi + (long long)(r - g) * nvp + j] = src[(g + nz - g + (r - g)) * nvp + j];           // my row nz-g+(r-g)
+  }
+}
+
 // the 6 velocity moments per z of a state (S1; Riemann sum of PAPER.md:78): one warp per z row,
 // lanes stride over v, fixed shuffle tree => reproducible.  mom[6][nz], already times dv.
 __global__ void moments_kernel(const double* __restrict__ y, double* __restrict__ mom, long long nz, int nv, int nvp,

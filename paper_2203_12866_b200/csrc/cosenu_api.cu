@@ -5,6 +5,8 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 
+#include <unistd.h>
+
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -41,6 +43,7 @@ struct cosenu {
   double eps_ko = 0.1, weno_eps = 1e-6;
   int advect = 1, rk_form = 2, stage_timing = 0;   // rk_form: 0 accumulator, 1 lean accumulator, 2 accumulator-free
   int quad = 0;          // COSENU_OPT_QUADRATURE
+  int ko_r = 2;          // COSENU_OPT_KO_ORDER: r of Eq. (5)
   double dz, dv, voff = 0.5;   // v_j = -1 + (j + voff) dv
   int device = 0;
   int variant = 0;       // kernel shape variant (COSENU_OPT_VARIANT)
@@ -68,6 +71,24 @@ struct cosenu {
   double stage_ms[4] = {0, 0, 0, 0}; int64_t stage_n = 0;
 
   std::set<const void*> configured;   // stage kernels whose shared-memory attribute is set on this device
+  bool dry_run = false;               // launch_one only sets the kernel attributes (before a stream capture)
+
+  // CUDA graph of GRAPH_STEPS RK4 steps (4 GRAPH_STEPS kernel nodes): replayed by cosenu_step when the launch
+  // parameters repeat from step to step (single domain, no per-stage events)
+  bool stream_owned = false;
+  int use_graph = 1;
+  cudaGraphExec_t gexec = nullptr;
+
+  // z-slab decomposition (cosenu_create_slab): this handle owns rows [z_begin, z_begin + nz) of nz_global
+  bool slab = false, linked = false, ghosts_pushed = false;
+  int64_t nz_global = 0, z_begin = 0;
+  unsigned long long* d_ctr = nullptr;   // my arrival counters: [0] low ghost rows, [1] high ghost rows
+  int* d_err = nullptr;                  // halo wait gave up
+  double* peer_buf[2][4] = {{nullptr, nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr, nullptr}};  // [lo|hi][U,Y1,Y2,ACC]
+  int64_t peer_stride[2] = {0, 0}, peer_nz[2] = {0, 0};
+  unsigned long long* peer_ctr[2] = {nullptr, nullptr};   // lo peer's HIGH counter, hi peer's LOW counter
+  void* ipc_mapped[2] = {nullptr, nullptr};               // bases returned by cudaIpcOpenMemHandle (closed in destroy)
+  unsigned long long epoch = 0;                           // stage launches since the link
 
   std::string err;
 };
@@ -87,7 +108,7 @@ int cuda_fail(cosenu* h, cudaError_t e, const char* what) {
     if (e_ != cudaSuccess) return cuda_fail(h, e_, #call);        \
   } while (0)
 
-size_t workspace_layout(const cosenu* h, size_t off[10]) {
+size_t workspace_layout(const cosenu* h, size_t off[11]) {
   const size_t st = align_up(sizeof(double) * 8 * (size_t)(h->nz + 2 * G) * h->nvp, 256);
   const size_t mo = align_up(sizeof(double) * 6 * (size_t)h->nz, 256);
   const size_t rf = align_up(sizeof(double) * 2 * (size_t)h->nv, 256);
@@ -104,6 +125,7 @@ size_t workspace_layout(const cosenu* h, size_t off[10]) {
   off[7] = o; o += rf;  // p0ref
   off[8] = o; o += rp;  // ref partials
   off[9] = o; o += dp;  // diag partials
+  off[10] = o; o += 256; // slab arrival counters (2 x u64) and the wait-failed flag (int, at +64)
   return o;
 }
 
@@ -121,10 +143,18 @@ int make_map(cosenu* h, PFN_encodeTiled enc, CUtensorMap* map, double* base, int
   return COSENU_OK;
 }
 
+int make_maps(cosenu* h);
+
 int ensure_workspace(cosenu* h) {
   if (h->maps_ready) return COSENU_OK;
   CK(cudaSetDevice(h->device));
-  size_t off[10];
+  if (!h->stream) {
+    // no caller stream: a BLOCKING stream of our own.  It orders with the legacy default stream exactly as
+    // default-stream work would (implicit synchronisation both ways), and unlike the legacy stream it can be captured.
+    CK(cudaStreamCreate(&h->stream));
+    h->stream_owned = true;
+  }
+  size_t off[11];
   const size_t need = workspace_layout(h, off);
   if (!h->ws) {
     cudaError_t e = cudaMalloc(&h->ws, need);
@@ -137,14 +167,23 @@ int ensure_workspace(cosenu* h) {
   h->M[0] = (double*)(b + off[4]); h->M[1] = (double*)(b + off[5]);
   h->d_pref = (double*)(b + off[6]); h->d_p0ref = (double*)(b + off[7]);
   h->d_refpart = (double*)(b + off[8]); h->d_diagpart = (double*)(b + off[9]);
+  h->d_ctr = (unsigned long long*)(b + off[10]); h->d_err = (int*)(b + off[10] + 64);
   CK(cudaMemsetAsync(h->ws, 0, need, h->stream));
 
+  int rc = make_maps(h);
+  if (rc) return rc;
+  h->maps_ready = true;
+  return COSENU_OK;
+}
+
+// halo of the stage-input boxes: 2 rows for FD4 + KO r = 2, 3 for KO r = 3, 4 for WENO7
+int make_maps(cosenu* h) {
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qr;
   CK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr));
   if (!fn || qr != cudaDriverEntryPointSuccess) return fail(h, COSENU_ECUDA, "cuTensorMapEncodeTiled not available in this driver");
   PFN_encodeTiled enc = reinterpret_cast<PFN_encodeTiled>(fn);
-  const int rows = TZ_ALL + 2 * (h->scheme == COSENU_FD4_KO3 ? 2 : 4);
+  const int rows = TZ_ALL + 2 * (h->scheme == COSENU_FD4_KO3 ? h->ko_r : 4);
   int rc;
   if ((rc = make_map(h, enc, &h->tm_U, h->U, rows, true))) return rc;
   if ((rc = make_map(h, enc, &h->tm_Y1, h->Y1, rows, true))) return rc;
@@ -154,7 +193,6 @@ int ensure_workspace(cosenu* h) {
   if ((rc = make_map(h, enc, &h->tp_Y1, h->Y1, TZ_ALL, false))) return rc;
   if ((rc = make_map(h, enc, &h->tp_Y2, h->Y2, TZ_ALL, false))) return rc;
   if ((rc = make_map(h, enc, &h->tp_ACC, h->ACC, TZ_ALL, false))) return rc;
-  h->maps_ready = true;
   return COSENU_OK;
 }
 
@@ -170,6 +208,7 @@ int launch_one(cosenu* h, const CUtensorMap& map, const CUtensorMap& omap, const
     CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     h->configured.insert(key);
   }
+  if (h->dry_run) return COSENU_OK;
   const long long ntiles = (h->nz + TZ - 1) / TZ;
   const unsigned grid = (unsigned)(ntiles < h->num_sms ? ntiles : h->num_sms);   // persistent: one CTA per SM
   kern<<<grid, NSEG * 32 + 32, smem, h->stream>>>(map, h->tp_U, a1, a2, omap, p);
@@ -184,7 +223,7 @@ int launch_kind(cosenu* h, int kind, const CUtensorMap& map, const CUtensorMap& 
   switch (kind) {
     case FIRST: return launch_one<SCHEME, FIRST, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
     // stage 1 of the lean forms loads nothing but the stage input: a deeper input ring keeps enough bytes in flight
-    case FIRST_LEAN: return launch_one<SCHEME, FIRST_LEAN, TZ, NSEG, (SCHEME == 0 ? 4 : NY), NUA>(h, map, omap, a1, a2, p);
+    case FIRST_LEAN: return launch_one<SCHEME, FIRST_LEAN, TZ, NSEG, (SCHEME == 0 ? 4 : (SCHEME == 2 ? 3 : NY)), NUA>(h, map, omap, a1, a2, p);
     case MID: return launch_one<SCHEME, MID, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
     case MID_REBUILD: return launch_one<SCHEME, MID_REBUILD, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
     case LAST: return launch_one<SCHEME, LAST, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
@@ -195,6 +234,10 @@ int launch_kind(cosenu* h, int kind, const CUtensorMap& map, const CUtensorMap& 
 
 int launch_stage(cosenu* h, int kind, const CUtensorMap& map, const CUtensorMap& omap, const CUtensorMap& a1,
                  const CUtensorMap& a2, const StageParams& p) {
+  if (h->scheme == COSENU_FD4_KO3 && h->ko_r == 3) {   // FD4 + Kreiss-Oliger r = 3: halo 3
+    if (h->variant == 1) return launch_kind<2, TZ_ALL, 16, 2, 2>(h, kind, map, omap, a1, a2, p);
+    return launch_kind<2, TZ_ALL, 8, 2, 2>(h, kind, map, omap, a1, a2, p);
+  }
   if (h->scheme == COSENU_FD4_KO3) {
     if (h->variant == 1) return launch_kind<0, TZ_ALL, 16, 2, 2>(h, kind, map, omap, a1, a2, p);
     return launch_kind<0, TZ_ALL, 8, 2, 2>(h, kind, map, omap, a1, a2, p);
@@ -213,7 +256,7 @@ StageParams base_params(const cosenu* h) {
   p.dv = h->dv; p.voff = h->voff; p.quad = h->quad;
   const double sw = h->advect ? 1.0 : 0.0;
   p.cadv = sw * (-1.0 / (12.0 * h->dz));
-  p.cko = sw * (-h->eps_ko / (16.0 * h->dz));
+  p.cko = h->ko_r == 3 ? sw * (h->eps_ko / (64.0 * h->dz)) : sw * (-h->eps_ko / (16.0 * h->dz));
   p.ninv_dz = sw * (-1.0 / h->dz);
   p.weno_eps = h->weno_eps;
   return p;
@@ -243,10 +286,73 @@ int drain_events(cosenu* h) {
   return COSENU_OK;
 }
 
-// one classical RK4 step = 4 fused stage launches.  Buffers: U -> Y1 -> Y2 -> Y1 -> U, accumulator ACC.
-int one_step(cosenu* h) {
+// y_out = state buffer `which` (0 U, 1 Y1, 2 Y2, 3 ACC) and where the ghost copies of its edge rows go:
+// my own periodic ghost rows, or (z-slab) the neighbouring slabs' ghost rows of the same buffer + the arrival counters
+void set_output(cosenu* h, StageParams& p, int which) {
+  double* bufs[4] = {h->U, h->Y1, h->Y2, h->ACC};
+  p.y_out = bufs[which];
+  if (!h->slab) {
+    p.ghost_lo_dst = p.y_out + (size_t)(h->nz + G) * h->nvp;   // rows 0..G-1 -> device rows nz+G.. (high ghosts)
+    p.ghost_hi_dst = p.y_out;                                    // rows nz-G..nz-1 -> device rows 0..G-1 (low ghosts)
+    p.ghost_lo_stride = p.ghost_hi_stride = h->comp_stride;
+    return;
+  }
+  // my low rows are the HIGH ghost rows of the slab below; my high rows are the LOW ghost rows of the slab above
+  p.ghost_lo_dst = h->peer_buf[0][which] + (size_t)(h->peer_nz[0] + G) * h->nvp;
+  p.ghost_lo_stride = h->peer_stride[0];
+  p.ghost_hi_dst = h->peer_buf[1][which];
+  p.ghost_hi_stride = h->peer_stride[1];
+  p.sig_lo = h->peer_ctr[0];
+  p.sig_hi = h->peer_ctr[1];
+  p.wait_lo = h->d_ctr;
+  p.wait_hi = h->d_ctr + 1;
+  p.wait_val = (unsigned long long)G * h->epoch;   // G rows per edge per stage launch so far
+  p.err_flag = h->d_err;
+  const long long ntiles = (h->nz + TZ_ALL - 1) / TZ_ALL;
+  p.tile_shift = ntiles >= 3 ? ntiles - 2 : 0;     // walk the (up to two) high edge tiles, then tile 0, first
+}
+
+// RK stage k (0..3) of the classical RK4 step = ONE fused launch.  Buffers: U -> Y1 -> Y2 -> (Y1 | ACC) -> U; in the
+// accumulator-free form the fourth state buffer (ACC) holds Y4, so that Y2 (in Y1) and Y3 (in Y2) are still there for
+// the final combination.  Moments ping-pong between M[mcur] (of U) and M[mcur ^ 1].
+int rk_stage(cosenu* h, int k) {
   const double dt = h->dt;
   StageParams p = base_params(h);
+  double* Min = h->M[h->mcur];
+  double* Mout = h->M[h->mcur ^ 1];
+  const int form = h->rk_form;
+  int rc = COSENU_OK;
+  switch (k) {
+    case 0:   // k1 = RHS(U); Y1 = U + dt/2 k1; [ACC = U + dt/6 k1]
+      set_output(h, p, 1); p.acc_out = h->ACC; p.mom_in = Min; p.mom_out = Mout;
+      p.cy = 0.5 * dt; p.ca = dt / 6.0;
+      rc = launch_stage(h, form == 0 ? FIRST : FIRST_LEAN, h->tm_U, h->tp_Y1, h->tp_ACC, h->tp_ACC, p);
+      break;
+    case 1:   // k2 = RHS(Y1); Y2 = U + dt/2 k2; [ACC += dt/3 k2]
+      set_output(h, p, 2); p.acc_out = h->ACC; p.mom_in = Mout; p.mom_out = Min;
+      p.cy = 0.5 * dt; p.ca = dt / 3.0;
+      rc = launch_stage(h, form == 0 ? MID : (form == 1 ? MID_REBUILD : MID_NOACC), h->tm_Y1, h->tp_Y2, h->tp_ACC,
+                        h->tp_ACC, p);
+      break;
+    case 2:   // k3 = RHS(Y2); Y4 = U + dt k3 (into Y1, or into ACC in the accumulator-free form); [ACC += dt/3 k3]
+      set_output(h, p, form == 2 ? 3 : 1); p.acc_out = h->ACC; p.mom_in = Min; p.mom_out = Mout;
+      p.cy = dt; p.ca = dt / 3.0;
+      rc = launch_stage(h, form == 2 ? MID_NOACC : MID, h->tm_Y2, form == 2 ? h->tp_ACC : h->tp_Y1, h->tp_ACC,
+                        h->tp_ACC, p);
+      break;
+    default:  // k4 = RHS(Y4); U = ACC + dt/6 k4   or   U = (Y2 + 2 Y3 + Y4 - U)/3 + dt/6 k4
+      set_output(h, p, 0); p.acc_out = nullptr; p.mom_in = Mout; p.mom_out = Min;
+      p.cy = dt / 6.0; p.ca = 0.0;
+      if (form == 2) rc = launch_stage(h, LAST_COMB, h->tm_ACC, h->tp_U, h->tp_Y1, h->tp_Y2, p);
+      else rc = launch_stage(h, LAST, h->tm_Y1, h->tp_U, h->tp_ACC, h->tp_ACC, p);
+      break;
+  }
+  if (rc == COSENU_OK && !h->dry_run) h->epoch++;
+  return rc;
+}
+
+// one classical RK4 step = 4 fused stage launches (the moments of the new U end up in M[mcur] again)
+int one_step(cosenu* h) {
   const bool tm = h->stage_timing != 0;
   int rc;
   cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
@@ -255,41 +361,50 @@ int one_step(cosenu* h) {
     for (int k = 0; k < 5; ++k) if (!(ev[k] = next_event(h))) return fail(h, COSENU_ECUDA, "cudaEventCreate failed");
     CK(cudaEventRecord(ev[0], h->stream));
   }
-  double* Min = h->M[h->mcur];
-  double* Mout = h->M[h->mcur ^ 1];
-  const int form = h->rk_form;
-  // buffers: U -> Y1 -> Y2 -> (Y1 | ACC) -> U.  In the accumulator-free form the fourth state buffer (ACC)
-  // holds Y4, so that Y2 (in Y1) and Y3 (in Y2) are still there for the final combination.
-  // stage 1: k1 = RHS(U); Y1 = U + dt/2 k1; [ACC = U + dt/6 k1]
-  p.y_out = h->Y1; p.acc_out = h->ACC; p.mom_in = Min; p.mom_out = Mout;
-  p.cy = 0.5 * dt; p.ca = dt / 6.0;
-  if ((rc = launch_stage(h, form == 0 ? FIRST : FIRST_LEAN, h->tm_U, h->tp_Y1, h->tp_ACC, h->tp_ACC, p))) return rc;
-  if (tm) CK(cudaEventRecord(ev[1], h->stream));
-  // stage 2: k2 = RHS(Y1); Y2 = U + dt/2 k2; [ACC += dt/3 k2]
-  p.y_out = h->Y2; p.acc_out = h->ACC; p.mom_in = Mout; p.mom_out = Min;
-  p.cy = 0.5 * dt; p.ca = dt / 3.0;
-  if ((rc = launch_stage(h, form == 0 ? MID : (form == 1 ? MID_REBUILD : MID_NOACC), h->tm_Y1, h->tp_Y2, h->tp_ACC,
-                         h->tp_ACC, p))) return rc;
-  if (tm) CK(cudaEventRecord(ev[2], h->stream));
-  // stage 3: k3 = RHS(Y2); Y4 = U + dt k3 (into Y1, or into ACC in the accumulator-free form); [ACC += dt/3 k3]
-  p.y_out = form == 2 ? h->ACC : h->Y1; p.mom_in = Min; p.mom_out = Mout;
-  p.cy = dt; p.ca = dt / 3.0;
-  if ((rc = launch_stage(h, form == 2 ? MID_NOACC : MID, h->tm_Y2, form == 2 ? h->tp_ACC : h->tp_Y1, h->tp_ACC,
-                         h->tp_ACC, p))) return rc;
-  if (tm) CK(cudaEventRecord(ev[3], h->stream));
-  // stage 4: k4 = RHS(Y4); U = ACC + dt/6 k4   or   U = (Y2 + 2 Y3 + Y4 - U)/3 + dt/6 k4
-  p.y_out = h->U; p.acc_out = nullptr; p.mom_in = Mout; p.mom_out = Min;
-  p.cy = dt / 6.0; p.ca = 0.0;
-  if (form == 2) rc = launch_stage(h, LAST_COMB, h->tm_ACC, h->tp_U, h->tp_Y1, h->tp_Y2, p);
-  else rc = launch_stage(h, LAST, h->tm_Y1, h->tp_U, h->tp_ACC, h->tp_ACC, p);
-  if (rc) return rc;
-  if (tm) CK(cudaEventRecord(ev[4], h->stream));
-  // moments of the new U are in Min = M[mcur] again
-  h->t += dt; h->step += 1;
+  for (int k = 0; k < 4; ++k) {
+    if ((rc = rk_stage(h, k))) return rc;
+    if (tm) CK(cudaEventRecord(ev[k + 1], h->stream));
+  }
+  h->t += h->dt; h->step += 1;
   return COSENU_OK;
 }
 
-int run_diag(cosenu* h, double sums[DIAG_NSUM], double maxs[DIAG_NMAX]) {
+// ---- diagnostics in four pieces, so that a decomposed run can put its reduction between them
+// (1) per-beam sums over my rows of |P_nu|, P0_nu, |P_nubar|, P0_nubar: out[4][nv]
+int ref_sums(cosenu* h, double* out) {
+  diag_ref_kernel<<<REF_BLOCKS, 256, 0, h->stream>>>(h->U, h->d_refpart, h->nz, h->nv, h->nvp, h->comp_stride, G);
+  CK(cudaGetLastError());
+  h->launches++;
+  std::vector<double> part((size_t)REF_BLOCKS * 4 * h->nv);
+  CK(cudaMemcpyAsync(part.data(), h->d_refpart, sizeof(double) * part.size(), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  for (int m = 0; m < 4; ++m)
+    for (int j = 0; j < h->nv; ++j) {
+      long double a = 0;
+      for (int b = 0; b < REF_BLOCKS; ++b) a += part[((size_t)b * 4 + m) * h->nv + j];
+      out[(size_t)m * h->nv + j] = (double)a;
+    }
+  return COSENU_OK;
+}
+// (2) the same sums over the whole grid -> references |P|_0(v), P0_0(v) = z-means at t = 0 (Eq. 22, 23)
+int set_ref_sums(cosenu* h, const double* sums) {
+  const int nv = h->nv;
+  const double nzg = (double)(h->slab ? h->nz_global : h->nz);
+  std::vector<double> pref(2 * (size_t)nv), p0ref(2 * (size_t)nv);
+  long double prsum = 0;
+  for (int j = 0; j < nv; ++j) {
+    pref[j] = sums[j] / nzg; p0ref[j] = sums[(size_t)nv + j] / nzg;
+    pref[nv + j] = sums[2 * (size_t)nv + j] / nzg; p0ref[nv + j] = sums[3 * (size_t)nv + j] / nzg;
+    prsum += (long double)quad_weight(j, nv, h->quad) * pref[j];
+  }
+  h->pref_sum_nu = (double)(prsum * nzg);
+  CK(cudaMemcpyAsync(h->d_pref, pref.data(), sizeof(double) * pref.size(), cudaMemcpyHostToDevice, h->stream));
+  CK(cudaMemcpyAsync(h->d_p0ref, p0ref.data(), sizeof(double) * p0ref.size(), cudaMemcpyHostToDevice, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  return COSENU_OK;
+}
+// (3) sums [0..6] and maxima [7..9] over my cells
+int diag_sums(cosenu* h, double* out10) {
   diag_kernel<<<DIAG_BLOCKS, DIAG_THREADS, 0, h->stream>>>(h->U, h->d_pref, h->d_p0ref, h->d_diagpart, h->nz, h->nv,
                                                            h->nvp, h->comp_stride, G, h->quad);
   CK(cudaGetLastError());
@@ -299,48 +414,59 @@ int run_diag(cosenu* h, double sums[DIAG_NSUM], double maxs[DIAG_NMAX]) {
   CK(cudaStreamSynchronize(h->stream));
   long double s[DIAG_NSUM];
   for (int k = 0; k < DIAG_NSUM; ++k) s[k] = 0;
-  for (int k = 0; k < DIAG_NMAX; ++k) maxs[k] = 0;
+  for (int k = 0; k < DIAG_NMAX; ++k) out10[DIAG_NSUM + k] = 0;
   for (int b = 0; b < DIAG_BLOCKS; ++b) {
     for (int k = 0; k < DIAG_NSUM; ++k) s[k] += part[(size_t)b * DIAG_NVAL + k];
-    for (int k = 0; k < DIAG_NMAX; ++k) maxs[k] = std::fmax(maxs[k], part[(size_t)b * DIAG_NVAL + DIAG_NSUM + k]);
+    for (int k = 0; k < DIAG_NMAX; ++k)
+      out10[DIAG_NSUM + k] = std::fmax(out10[DIAG_NSUM + k], part[(size_t)b * DIAG_NVAL + DIAG_NSUM + k]);
   }
-  for (int k = 0; k < DIAG_NSUM; ++k) sums[k] = (double)s[k];
+  for (int k = 0; k < DIAG_NSUM; ++k) out10[k] = (double)s[k];
   return COSENU_OK;
+}
+// (4) whole-grid sums / maxima -> the diagnostics; set_reference stores the t = 0 values
+void diag_finish(cosenu* h, const double* g, int set_reference, cosenu_diag_t* d) {
+  const double* sums = g;
+  const double* maxs = g + DIAG_NSUM;
+  if (set_reference) {
+    h->sum_ee0[0] = sums[0]; h->sum_ee0[1] = sums[1];
+    for (int m = 0; m < 3; ++m) h->M0_init[m] = sums[3 + m] * (h->dz * h->dv);
+  }
+  if (!d) return;
+  d->t = h->t; d->step = h->step;
+  d->psurv_nu = h->sum_ee0[0] != 0 ? sums[0] / h->sum_ee0[0] : 0.0;
+  d->psurv_nubar = h->sum_ee0[1] != 0 ? sums[1] / h->sum_ee0[1] : 0.0;
+  d->dP_max = maxs[0];
+  d->dP_avg = h->pref_sum_nu > 0 ? sums[2] / h->pref_sum_nu : 0.0;
+  for (int m = 0; m < 3; ++m) { d->M0[m] = sums[3 + m] * (h->dz * h->dv); d->dM0[m] = d->M0[m] - h->M0_init[m]; }
+  d->trace_dev_max = maxs[1];
+  d->ex_abs_max = maxs[2];
 }
 
 // after U has been uploaded: ghosts, moments, diagnostic references
 int finish_upload(cosenu* h, double t) {
-  fill_ghosts_kernel<<<64, 256, 0, h->stream>>>(h->U, h->nz, h->nvp, h->comp_stride, G);
-  CK(cudaGetLastError());
-  h->mcur = 0;
-  moments_kernel<<<592, 256, 0, h->stream>>>(h->U, h->M[0], h->nz, h->nv, h->nvp, h->comp_stride, G, h->dv, h->voff, h->quad);
-  CK(cudaGetLastError());
-  diag_ref_kernel<<<REF_BLOCKS, 256, 0, h->stream>>>(h->U, h->d_refpart, h->nz, h->nv, h->nvp, h->comp_stride, G);
-  CK(cudaGetLastError());
-  h->launches += 3;
-  std::vector<double> part((size_t)REF_BLOCKS * 4 * h->nv);
-  CK(cudaMemcpyAsync(part.data(), h->d_refpart, sizeof(double) * part.size(), cudaMemcpyDeviceToHost, h->stream));
-  CK(cudaStreamSynchronize(h->stream));
-  std::vector<double> pref(2 * (size_t)h->nv), p0ref(2 * (size_t)h->nv);
-  long double prsum = 0;
-  for (int j = 0; j < h->nv; ++j) {
-    long double a[4] = {0, 0, 0, 0};
-    for (int b = 0; b < REF_BLOCKS; ++b)
-      for (int m = 0; m < 4; ++m) a[m] += part[((size_t)b * 4 + m) * h->nv + j];
-    pref[j] = (double)(a[0] / h->nz); p0ref[j] = (double)(a[1] / h->nz);
-    pref[h->nv + j] = (double)(a[2] / h->nz); p0ref[h->nv + j] = (double)(a[3] / h->nz);
-    prsum += (long double)quad_weight(j, h->nv, h->quad) * pref[j];
+  if (!h->slab) {
+    fill_ghosts_kernel<<<64, 256, 0, h->stream>>>(h->U, h->nz, h->nvp, h->comp_stride, G);
+    CK(cudaGetLastError());
+    h->launches++;
   }
-  h->pref_sum_nu = (double)(prsum * h->nz);
-  CK(cudaMemcpyAsync(h->d_pref, pref.data(), sizeof(double) * pref.size(), cudaMemcpyHostToDevice, h->stream));
-  CK(cudaMemcpyAsync(h->d_p0ref, p0ref.data(), sizeof(double) * p0ref.size(), cudaMemcpyHostToDevice, h->stream));
-  CK(cudaStreamSynchronize(h->stream));
-  double sums[DIAG_NSUM], maxs[DIAG_NMAX];
-  int rc = run_diag(h, sums, maxs);
-  if (rc) return rc;
-  h->sum_ee0[0] = sums[0]; h->sum_ee0[1] = sums[1];
-  for (int m = 0; m < 3; ++m) h->M0_init[m] = sums[3 + m] * (h->dz * h->dv);
+  h->mcur = 0;
+  moments_kernel<<<592, 256, 0, h->stream>>>(h->U, h->M[0], h->nz, h->nv, h->nvp, h->comp_stride, G, h->dv, h->voff,
+                                             h->quad);
+  CK(cudaGetLastError());
+  h->launches++;
   h->t = t; h->step = 0; h->have_state = true;
+  if (h->slab) {   // ghost rows and references need the other slabs: slab_push_ghosts, slab_*_sums
+    h->ghosts_pushed = false;
+    CK(cudaStreamSynchronize(h->stream));
+    return COSENU_OK;
+  }
+  std::vector<double> rs(4 * (size_t)h->nv);
+  int rc;
+  if ((rc = ref_sums(h, rs.data()))) return rc;
+  if ((rc = set_ref_sums(h, rs.data()))) return rc;
+  double g[DIAG_NVAL];
+  if ((rc = diag_sums(h, g))) return rc;
+  diag_finish(h, g, 1, nullptr);
   return COSENU_OK;
 }
 
@@ -353,11 +479,43 @@ inline uint64_t splitmix64_next(uint64_t& s) {
 
 }  // namespace
 
+namespace {
+constexpr int GRAPH_STEPS = 8;
+
+void drop_graph(cosenu* h) {
+  if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
+}
+
+// capture GRAPH_STEPS steps of the current configuration into an executable graph
+int build_graph(cosenu* h) {
+  h->dry_run = true;                     // kernel attributes first: nothing but launches inside the capture
+  for (int k = 0; k < 4; ++k) { int rc = rk_stage(h, k); if (rc) { h->dry_run = false; return rc; } }
+  h->dry_run = false;
+  const int64_t launches0 = h->launches, step0 = h->step;
+  const double t0 = h->t;
+  const unsigned long long epoch0 = h->epoch;
+  CK(cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
+  int rc = COSENU_OK;
+  for (int s = 0; s < GRAPH_STEPS && rc == COSENU_OK; ++s) rc = one_step(h);
+  cudaGraph_t graph = nullptr;
+  cudaError_t e = cudaStreamEndCapture(h->stream, &graph);
+  h->launches = launches0; h->step = step0; h->t = t0; h->epoch = epoch0;   // nothing has run yet
+  if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+  if (e != cudaSuccess) return cuda_fail(h, e, "cudaStreamEndCapture");
+  e = cudaGraphInstantiate(&h->gexec, graph, 0);
+  cudaGraphDestroy(graph);
+  if (e != cudaSuccess) { h->gexec = nullptr; return cuda_fail(h, e, "cudaGraphInstantiate"); }
+  return COSENU_OK;
+}
+}  // namespace
+
 // ================================================================================ C ABI
-extern "C" cosenu_t* cosenu_create(int64_t nz, int32_t nv, double L, double dt, double omega, double theta, double mu,
-                                   int scheme) {
-  if (nz < 16 || nz > 2000000000ll || nv < 2 || nv > (1 << 20) || !(L > 0) || !(dt > 0) || (scheme != 0 && scheme != 1) ||
-      !std::isfinite(L) || !std::isfinite(dt) || !std::isfinite(omega) || !std::isfinite(theta) || !std::isfinite(mu)) {
+namespace {
+cosenu* create_common(int64_t nz_global, int64_t z_begin, int64_t nz, int32_t nv, double L, double dt, double omega,
+                      double theta, double mu, int scheme, bool slab) {
+  if (nz < 16 || nz > 2000000000ll || nz_global < nz || nz_global > 2000000000ll || z_begin < 0 || z_begin >= nz_global ||
+      nv < 2 || nv > (1 << 20) || !(L > 0) || !(dt > 0) || (scheme != 0 && scheme != 1) || !std::isfinite(L) ||
+      !std::isfinite(dt) || !std::isfinite(omega) || !std::isfinite(theta) || !std::isfinite(mu)) {
     g_create_err = "cosenu_create: invalid argument";
     return nullptr;
   }
@@ -375,17 +533,29 @@ extern "C" cosenu_t* cosenu_create(int64_t nz, int32_t nv, double L, double dt, 
   cosenu* h = new (std::nothrow) cosenu();
   if (!h) { g_create_err = "out of memory"; return nullptr; }
   h->nz = nz; h->nv = nv; h->L = L; h->dt = dt; h->omega = omega; h->theta = theta; h->mu = mu; h->scheme = scheme;
+  h->slab = slab; h->nz_global = nz_global; h->z_begin = z_begin;
   h->device = dev;
   h->nvp = (nv + 3) / 4 * 4;
-  h->dz = L / (double)nz; h->dv = 2.0 / (double)nv;
+  h->dz = L / (double)nz_global; h->dv = 2.0 / (double)nv;
   h->comp_stride = (int64_t)(nz + 2 * G) * h->nvp;
   h->num_sms = prop.multiProcessorCount;
   return h;
 }
+}  // namespace
+
+extern "C" cosenu_t* cosenu_create(int64_t nz, int32_t nv, double L, double dt, double omega, double theta, double mu,
+                                   int scheme) {
+  return create_common(nz, 0, nz, nv, L, dt, omega, theta, mu, scheme, false);
+}
+
+extern "C" cosenu_t* cosenu_create_slab(int64_t nz_global, int64_t z_begin, int64_t nz_local, int32_t nv, double L,
+                                        double dt, double omega, double theta, double mu, int scheme) {
+  return create_common(nz_global, z_begin, nz_local, nv, L, dt, omega, theta, mu, scheme, true);
+}
 
 extern "C" size_t cosenu_workspace_bytes(const cosenu_t* h) {
   if (!h) return 0;
-  size_t off[10];
+  size_t off[11];
   return workspace_layout(h, off);
 }
 
@@ -403,12 +573,21 @@ extern "C" int cosenu_attach(cosenu_t* h, void* dev_workspace, size_t bytes, voi
 
 extern "C" int cosenu_set_option(cosenu_t* h, int key, double value) {
   if (!h) return COSENU_EINVAL;
+  drop_graph(h);   // the captured launch parameters may change
   switch (key) {
+    case COSENU_OPT_GRAPH: h->use_graph = value != 0; return COSENU_OK;
     case COSENU_OPT_EPS_KO: if (!(value >= 0) || !std::isfinite(value)) break; h->eps_ko = value; return COSENU_OK;
     case COSENU_OPT_WENO_EPS: if (!(value > 0) || !(value <= 1e30)) break; h->weno_eps = value; return COSENU_OK;
     case COSENU_OPT_ADVECT: h->advect = value != 0; return COSENU_OK;
     case COSENU_OPT_RK_FORM: if (value != 0 && value != 1 && value != 2) break; h->rk_form = (int)value; return COSENU_OK;
     case COSENU_OPT_VARIANT: if (value != 0 && value != 1) break; h->variant = (int)value; return COSENU_OK;
+    case COSENU_OPT_KO_ORDER:
+      if (value != 2 && value != 3) break;
+      if (h->ko_r != (int)value) {
+        h->ko_r = (int)value;
+        if (h->maps_ready) { int rc = make_maps(h); if (rc) return rc; }   // the stage-input boxes carry the halo
+      }
+      return COSENU_OK;
     case COSENU_OPT_QUADRATURE:
       if ((value != 0 && value != 1 && value != 2) || (value == 2 && (h->nv % 2 == 0 || h->nv < 3))) break;
       if (h->have_state) return fail(h, COSENU_ESTATE, "cosenu_set_option: the quadrature must be chosen before init / set_state");
@@ -460,8 +639,11 @@ extern "C" int cosenu_init(cosenu_t* h, uint64_t seed, double sigma_nu, double s
   for (int j = 0; j < nv; ++j) { g[j] = g[j] / (sg * h->dv); gb[j] = alpha * (gb[j] / (sgb * h->dv)); }
   const double two_pi = 6.283185307179586476925286766559;
   std::vector<double> pr(nz), pi(nz), dd(nz, 1.0);
+  // a slab builds its own rows of the global initial state: global row zg = z_begin + i of nzg rows
+  const int64_t z0 = h->z_begin, nzg = h->nz_global;
   uint64_t s = seed;
   if (pert_kind == 0) {
+    s += (uint64_t)z0 * 0x9E3779B97F4A7C15ull;   // splitmix64's state advances by a constant per draw: skip z0 draws
     for (int64_t i = 0; i < nz; ++i) {
       const double u = (double)(splitmix64_next(s) >> 11) * (1.0 / 9007199254740992.0);
       pr[i] = pert_amp * std::cos(two_pi * u); pi[i] = pert_amp * std::sin(two_pi * u);
@@ -472,14 +654,14 @@ extern "C" int cosenu_init(cosenu_t* h, uint64_t seed, double sigma_nu, double s
     for (int64_t i = 0; i < nz; ++i) {
       double a = 0, b = 0;
       for (int q = 0; q < K; ++q) {
-        const double arg = two_pi * (double)(q + 1) * (double)i / (double)nz + ph[q];
+        const double arg = two_pi * (double)(q + 1) * (double)(z0 + i) / (double)nzg + ph[q];
         a += std::cos(arg); b += std::sin(arg);
       }
       pr[i] = pert_amp * a / 4.0; pi[i] = pert_amp * b / 4.0;
     }
   } else {
     for (int64_t i = 0; i < nz; ++i) {
-      const double zc = (h->scheme == COSENU_FV_WENO7 ? (i + 0.5) : (double)i) * h->dz - 0.5 * h->L;
+      const double zc = (h->scheme == COSENU_FV_WENO7 ? ((z0 + i) + 0.5) : (double)(z0 + i)) * h->dz - 0.5 * h->L;
       const double e = pert_amp * std::exp(-zc * zc / 50.0);
       pr[i] = 0.5 * e; pi[i] = 0.0; dd[i] = std::sqrt(1.0 - e * e);
     }
@@ -499,7 +681,19 @@ extern "C" int cosenu_init(cosenu_t* h, uint64_t seed, double sigma_nu, double s
 extern "C" int cosenu_step(cosenu_t* h, int64_t n) {
   if (!h || n < 0) return h ? fail(h, COSENU_EINVAL, "cosenu_step: n < 0") : COSENU_EINVAL;
   if (!h->have_state) return fail(h, COSENU_ESTATE, "cosenu_step: no state, call cosenu_init or cosenu_set_state first");
+  if (h->slab && !(h->linked && h->ghosts_pushed))
+    return fail(h, COSENU_ESTATE, "cosenu_step: a slab must be linked (cosenu_slab_link) and its ghost rows exchanged "
+                                  "(cosenu_slab_push_ghosts) first");
   CK(cudaSetDevice(h->device));
+  if (h->use_graph && !h->slab && !h->stage_timing && n >= 2 * GRAPH_STEPS) {
+    if (!h->gexec) { int rc = build_graph(h); if (rc) return rc; }
+    for (; n >= GRAPH_STEPS; n -= GRAPH_STEPS) {
+      CK(cudaGraphLaunch(h->gexec, h->stream));
+      h->launches += 4 * GRAPH_STEPS; h->epoch += 4 * GRAPH_STEPS;
+      h->step += GRAPH_STEPS;
+      for (int s = 0; s < GRAPH_STEPS; ++s) h->t += h->dt;   // same rounding as step-by-step accumulation
+    }
+  }
   for (int64_t s = 0; s < n; ++s) {
     int rc = one_step(h);
     if (rc) return rc;
@@ -536,17 +730,12 @@ extern "C" int cosenu_get_moments(cosenu_t* h, double* host_out) {
 extern "C" int cosenu_diagnostics(cosenu_t* h, cosenu_diag_t* d) {
   if (!h || !d) return COSENU_EINVAL;
   if (!h->have_state) return fail(h, COSENU_ESTATE, "cosenu_diagnostics: no state");
-  double sums[DIAG_NSUM], maxs[DIAG_NMAX];
-  int rc = run_diag(h, sums, maxs);
+  if (h->slab) return fail(h, COSENU_ESTATE, "cosenu_diagnostics: a slab holds part of the grid; use cosenu_slab_diag_sums + "
+                                             "a reduction over the slabs + cosenu_slab_diag_finish");
+  double g[DIAG_NVAL];
+  int rc = diag_sums(h, g);
   if (rc) return rc;
-  d->t = h->t; d->step = h->step;
-  d->psurv_nu = h->sum_ee0[0] != 0 ? sums[0] / h->sum_ee0[0] : 0.0;
-  d->psurv_nubar = h->sum_ee0[1] != 0 ? sums[1] / h->sum_ee0[1] : 0.0;
-  d->dP_max = maxs[0];
-  d->dP_avg = h->pref_sum_nu > 0 ? sums[2] / h->pref_sum_nu : 0.0;
-  for (int m = 0; m < 3; ++m) { d->M0[m] = sums[3 + m] * (h->dz * h->dv); d->dM0[m] = d->M0[m] - h->M0_init[m]; }
-  d->trace_dev_max = maxs[1];
-  d->ex_abs_max = maxs[2];
+  diag_finish(h, g, 0, d);
   return COSENU_OK;
 }
 
@@ -566,8 +755,168 @@ extern "C" void cosenu_destroy(cosenu_t* h) {
   cudaSetDevice(h->device);
   if (h->maps_ready) cudaStreamSynchronize(h->stream);
   for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
+  drop_graph(h);
+  for (int k = 0; k < 2; ++k)
+    if (h->ipc_mapped[k] && (k == 0 || h->ipc_mapped[1] != h->ipc_mapped[0])) cudaIpcCloseMemHandle(h->ipc_mapped[k]);
   if (h->ws_owned && h->ws) cudaFree(h->ws);
+  if (h->stream_owned) cudaStreamDestroy(h->stream);
   delete h;
 }
 
 extern "C" const char* cosenu_last_error(const cosenu_t* h) { return h ? h->err.c_str() : g_create_err.c_str(); }
+
+// ================================================================================ z-slab decomposition
+namespace {
+typedef CUresult (*PFN_getAddressRange)(CUdeviceptr*, size_t*, CUdeviceptr);
+}
+
+extern "C" int cosenu_slab_export(cosenu_t* h, cosenu_slab_peer_t* out) {
+  if (!h || !out) return COSENU_EINVAL;
+  if (!h->slab) return fail(h, COSENU_ESTATE, "cosenu_slab_export: not a slab handle (cosenu_create_slab)");
+  int rc = ensure_workspace(h);
+  if (rc) return rc;
+  CK(cudaStreamSynchronize(h->stream));   // the workspace is zeroed (counters start at 0) before anybody can reach it
+  std::memset(out, 0, sizeof(*out));
+  // the IPC handle names the whole allocation: find its base (a caller-owned workspace may sit inside a larger one)
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qr;
+  CK(cudaGetDriverEntryPoint("cuMemGetAddressRange", &fn, cudaEnableDefault, &qr));
+  CUdeviceptr base = 0; size_t size = 0;
+  if (!fn || qr != cudaDriverEntryPointSuccess ||
+      reinterpret_cast<PFN_getAddressRange>(fn)(&base, &size, (CUdeviceptr)h->ws) != CUDA_SUCCESS)
+    return fail(h, COSENU_ECUDA, "cosenu_slab_export: cuMemGetAddressRange failed");
+  cudaIpcMemHandle_t ipc;
+  cudaError_t e = cudaIpcGetMemHandle(&ipc, (void*)base);
+  if (e == cudaSuccess) {
+    static_assert(sizeof(ipc) == 64, "cudaIpcMemHandle_t");
+    std::memcpy(out->ipc_handle, &ipc, 64);
+  } else {
+    (void)cudaGetLastError();   // not shareable (e.g. a pooled allocation): the slab can still be linked inside this process
+  }
+  out->ipc_offset = (uint64_t)((CUdeviceptr)h->ws - base);
+  out->dev_base = (uint64_t)(uintptr_t)h->ws;
+  out->pid = (int64_t)getpid();
+  out->device = h->device;
+  out->nvp = h->nvp;
+  out->nz_local = h->nz;
+  out->comp_stride = h->comp_stride;
+  const char* b = static_cast<const char*>(h->ws);
+  out->off_buf[0] = (uint64_t)((const char*)h->U - b); out->off_buf[1] = (uint64_t)((const char*)h->Y1 - b);
+  out->off_buf[2] = (uint64_t)((const char*)h->Y2 - b); out->off_buf[3] = (uint64_t)((const char*)h->ACC - b);
+  out->off_ctr = (uint64_t)((const char*)h->d_ctr - b);
+  return COSENU_OK;
+}
+
+extern "C" int cosenu_slab_link(cosenu_t* h, const cosenu_slab_peer_t* lo, const cosenu_slab_peer_t* hi) {
+  if (!h || !lo || !hi) return COSENU_EINVAL;
+  if (!h->slab) return fail(h, COSENU_ESTATE, "cosenu_slab_link: not a slab handle");
+  if (h->linked) return fail(h, COSENU_ESTATE, "cosenu_slab_link: already linked");
+  int rc = ensure_workspace(h);
+  if (rc) return rc;
+  const cosenu_slab_peer_t* peers[2] = {lo, hi};
+  for (int k = 0; k < 2; ++k) {
+    const cosenu_slab_peer_t* q = peers[k];
+    if (q->nvp != h->nvp || q->nz_local < 16) return fail(h, COSENU_EINVAL, "cosenu_slab_link: neighbour has another v-grid or is too thin");
+    char* base = nullptr;
+    if (q->pid == (int64_t)getpid()) {
+      base = reinterpret_cast<char*>((uintptr_t)q->dev_base);
+      if (q->device != h->device) {   // another GPU of this process: direct peer access
+        cudaError_t e = cudaDeviceEnablePeerAccess(q->device, 0);
+        if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled) return cuda_fail(h, e, "cudaDeviceEnablePeerAccess");
+        (void)cudaGetLastError();
+      }
+    } else if (k == 1 && lo->pid == hi->pid && std::memcmp(lo->ipc_handle, hi->ipc_handle, 64) == 0 && h->ipc_mapped[0]) {
+      h->ipc_mapped[1] = h->ipc_mapped[0];   // two slabs in a ring: both neighbours are the same allocation
+      base = static_cast<char*>(h->ipc_mapped[1]) + q->ipc_offset;
+    } else {
+      cudaIpcMemHandle_t ipc;
+      std::memcpy(&ipc, q->ipc_handle, 64);
+      void* mapped = nullptr;
+      cudaError_t e = cudaIpcOpenMemHandle(&mapped, ipc, cudaIpcMemLazyEnablePeerAccess);
+      if (e != cudaSuccess) return cuda_fail(h, e, "cudaIpcOpenMemHandle (neighbouring slab)");
+      h->ipc_mapped[k] = mapped;
+      base = static_cast<char*>(mapped) + q->ipc_offset;
+    }
+    for (int b = 0; b < 4; ++b) h->peer_buf[k][b] = reinterpret_cast<double*>(base + q->off_buf[b]);
+    h->peer_stride[k] = q->comp_stride;
+    h->peer_nz[k] = q->nz_local;
+    // my low rows land in the lower slab's HIGH ghost rows (its counter [1]); my high rows in the upper slab's LOW ones ([0])
+    h->peer_ctr[k] = reinterpret_cast<unsigned long long*>(base + q->off_ctr) + (k == 0 ? 1 : 0);
+  }
+  h->linked = true;
+  h->epoch = 0;
+  return COSENU_OK;
+}
+
+extern "C" int cosenu_slab_push_ghosts(cosenu_t* h) {
+  if (!h) return COSENU_EINVAL;
+  if (!h->slab || !h->linked) return fail(h, COSENU_ESTATE, "cosenu_slab_push_ghosts: slab not linked");
+  if (!h->have_state) return fail(h, COSENU_ESTATE, "cosenu_slab_push_ghosts: no state");
+  CK(cudaSetDevice(h->device));
+  push_ghosts_kernel<<<64, 256, 0, h->stream>>>(h->U, h->nz, h->nvp, h->comp_stride, G,
+                                                h->peer_buf[0][0] + (size_t)(h->peer_nz[0] + G) * h->nvp, h->peer_stride[0],
+                                                h->peer_buf[1][0], h->peer_stride[1]);
+  CK(cudaGetLastError());
+  h->launches++;
+  CK(cudaStreamSynchronize(h->stream));
+  h->ghosts_pushed = true;
+  return COSENU_OK;
+}
+
+extern "C" int cosenu_slab_ref_sums(cosenu_t* h, double* out) {
+  if (!h || !out) return COSENU_EINVAL;
+  if (!h->have_state) return fail(h, COSENU_ESTATE, "cosenu_slab_ref_sums: no state");
+  return ref_sums(h, out);
+}
+
+extern "C" int cosenu_slab_set_ref_sums(cosenu_t* h, const double* global_sums) {
+  if (!h || !global_sums) return COSENU_EINVAL;
+  if (!h->have_state) return fail(h, COSENU_ESTATE, "cosenu_slab_set_ref_sums: no state");
+  return set_ref_sums(h, global_sums);
+}
+
+extern "C" int cosenu_slab_diag_sums(cosenu_t* h, double* out10) {
+  if (!h || !out10) return COSENU_EINVAL;
+  if (!h->have_state) return fail(h, COSENU_ESTATE, "cosenu_slab_diag_sums: no state");
+  return diag_sums(h, out10);
+}
+
+extern "C" int cosenu_slab_diag_finish(cosenu_t* h, const double* global10, int set_reference, cosenu_diag_t* out) {
+  if (!h || !global10) return COSENU_EINVAL;
+  if (!h->have_state) return fail(h, COSENU_ESTATE, "cosenu_slab_diag_finish: no state");
+  diag_finish(h, global10, set_reference, out);
+  return COSENU_OK;
+}
+
+extern "C" int cosenu_slab_step_group(cosenu_t** hs, int32_t count, int64_t n) {
+  if (!hs || count < 1 || n < 0) return COSENU_EINVAL;
+  for (int i = 0; i < count; ++i) {
+    cosenu* h = hs[i];
+    if (!h) return COSENU_EINVAL;
+    if (!h->slab || !h->linked || !h->ghosts_pushed || !h->have_state)
+      return fail(h, COSENU_ESTATE, "cosenu_slab_step_group: every slab must be linked, hold a state and have its ghosts exchanged");
+    if (h->stream != hs[0]->stream || h->device != hs[0]->device)
+      return fail(h, COSENU_EINVAL, "cosenu_slab_step_group: the slabs of a group share one device and one stream");
+  }
+  cudaError_t e = cudaSetDevice(hs[0]->device);
+  if (e != cudaSuccess) return cuda_fail(hs[0], e, "cudaSetDevice");
+  for (int64_t s = 0; s < n; ++s) {
+    for (int k = 0; k < 4; ++k)
+      for (int i = 0; i < count; ++i) {
+        int rc = rk_stage(hs[i], k);
+        if (rc) return rc;
+      }
+    for (int i = 0; i < count; ++i) { hs[i]->t += hs[i]->dt; hs[i]->step += 1; }
+  }
+  return COSENU_OK;
+}
+
+extern "C" int cosenu_slab_wait_failed(cosenu_t* h, int32_t* failed) {
+  if (!h || !failed) return COSENU_EINVAL;
+  if (!h->maps_ready) { *failed = 0; return COSENU_OK; }
+  int v = 0;
+  CK(cudaMemcpyAsync(&v, h->d_err, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  *failed = v;
+  return COSENU_OK;
+}

@@ -17,3 +17,7 @@ extern "C" void cosenu_probe_weno7_face2(const double* w8, double v, double eps,
 extern "C" double cosenu_probe_fd4_ko3(const double* u5, double v, double dz, double eps_ko) {
   return cosenu_math::fd4_ko3(u5[0], u5[1], u5[2], u5[3], u5[4], -v / (12.0 * dz), -eps_ko / (16.0 * dz));
 }
+
+extern "C" double cosenu_probe_fd4_ko5(const double* u7, double v, double dz, double eps_ko) {
+  return cosenu_math::fd4_ko5(u7[0], u7[1], u7[2], u7[3], u7[4], u7[5], u7[6], -v / (12.0 * dz), eps_ko / (64.0 * dz));
+}

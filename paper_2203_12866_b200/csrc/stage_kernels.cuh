@@ -52,8 +52,25 @@ struct StageParams {
   double mu, A0, Br0;     // A0 = -omega cos 2theta, Br0 = (omega/2) sin 2theta
   double dv, voff;         // v_j = -1 + (j + voff) dv: voff = 1/2 bin centres, 0 vertex-centred
   int quad;                // rule of the v' integral: 0 Riemann/midpoint, 1 trapezoid, 2 Simpson (aux_kernels.cuh: quad_weight)
-  double cadv, cko;          // FD: -1/(12 dz), -eps_ko/(16 dz)   (times the advect switch)
+  double cadv, cko;          // FD: -1/(12 dz), -eps_ko/(16 dz) [KO r = 2] or +eps_ko/(64 dz) [r = 3]  (times the advect switch)
   double ninv_dz, weno_eps;  // WENO: -1/dz (times the advect switch), epsilon of Eq. (14)
+  // ---- ghost rows of y_out.  The copies of my first / last G rows go to
+  //   ghost_lo_dst[c * ghost_lo_stride + iz * nvp + j]              (iz = 0..G-1)
+  //   ghost_hi_dst[c * ghost_hi_stride + (iz - (nz - G)) * nvp + j] (iz = nz-G..nz-1)
+  // single periodic domain: my own ghost rows; z-slab: the neighbouring slabs' ghost rows (peer memory).
+  double* ghost_lo_dst;
+  double* ghost_hi_dst;
+  long long ghost_lo_stride, ghost_hi_stride;
+  // z-slab only (null otherwise): arrival counters, in rows.  sig_*: the neighbours' counters, bumped (release, system
+  // scope) once the ghost rows written above are visible; wait_*: my own counters, which must have reached wait_val
+  // before a tile that touches the low / high ghost rows of the stage input is loaded.
+  unsigned long long* sig_lo;
+  unsigned long long* sig_hi;
+  const unsigned long long* wait_lo;
+  const unsigned long long* wait_hi;
+  unsigned long long wait_val;
+  int* err_flag;           // set to 1 when a wait gives up (a neighbour that never arrives must not hang the GPU)
+  long long tile_shift;    // the l-th tile a CTA grid walks is tile (l + tile_shift) mod ntiles (slab: edge tiles first)
 };
 
 // ----------------------------------------------------------------------------- PTX helpers
@@ -109,6 +126,33 @@ __device__ __forceinline__ void sts(uint32_t addr, double v) {
   asm volatile("st.shared.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory");
 }
 
+// ---- cross-GPU arrival counters (z-slab halo exchange)
+__device__ __forceinline__ unsigned long long ld_acquire_sys(const unsigned long long* p) {
+  unsigned long long v;
+  asm volatile("ld.acquire.sys.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void red_add_release_sys(unsigned long long* p, unsigned long long v) {
+  asm volatile("red.release.sys.global.add.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ unsigned long long global_timer_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
+// wait until *ctr >= val; gives up after ~4 s (sets *err) so that a missing neighbour is an error, not a hang
+__device__ __noinline__ void wait_arrivals(const unsigned long long* ctr, unsigned long long val, int* err) {
+  if (ld_acquire_sys(ctr) >= val) return;
+  const unsigned long long t0 = global_timer_ns();
+  while (ld_acquire_sys(ctr) < val) {
+    __nanosleep(200);
+    if (global_timer_ns() - t0 > 4000000000ull) {
+      if (err) atomicExch(err, 1);
+      return;
+    }
+  }
+}
+
 template <int KIND>
 struct KindTraits {
   static constexpr bool LOAD_U0 = (KIND == MID || KIND == MID_REBUILD || KIND == MID_NOACC || KIND == LAST_COMB);
@@ -125,7 +169,7 @@ struct KindTraits {
 // shared-memory carve-up (byte offsets from a 128-byte aligned base)
 template <int SCHEME, int KIND, int TZ, int NSEG, int NY, int NUA>
 struct StageSmem {
-  static constexpr int H = SCHEME == 0 ? 2 : 4;
+  static constexpr int H = SCHEME == 0 ? 2 : (SCHEME == 1 ? 4 : 3);   // SCHEME 2 = FD4 + KO of order r = 3
   static constexpr int ROWS = TZ + 2 * H;
   static constexpr uint32_t YTILE = 8u * ROWS * VC * 8u;   // bytes per stage-input slot
   static constexpr uint32_t PTILE = 8u * TZ * VC * 8u;     // bytes per staging array
@@ -244,7 +288,7 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
   constexpr int NW = NSEG;  // compute warps
   constexpr int NARR = KT::NARR;
   static_assert(TZ % NSEG == 0 && 6 * S <= 32, "tile shape");
-  static_assert(SCHEME == 0 || NSEG >= 8, "WENO boundary flux is split over 8 warps");
+  static_assert(SCHEME != 1 || NSEG >= 8, "WENO boundary flux is split over 8 warps");
 
   extern __shared__ unsigned char smem_raw[];
   const uint32_t sbase = (smem_u32(smem_raw) + 127u) & ~127u;
@@ -263,6 +307,8 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
   const long long ntiles = (p.nz + TZ - 1) / TZ;
   const long long my_tiles = blockIdx.x < ntiles ? (ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
   const long long nitems = my_tiles * nchunks;
+  // the l-th tile of the walk (l = blockIdx.x + k gridDim.x < ntiles)
+  auto tile_of = [&](long long l) { const long long t = l + p.tile_shift; return t >= ntiles ? t - ntiles : t; };
 
   if (threadIdx.x == 0) {
     for (int b = 0; b < NY; ++b) { mbar_init(b_full_y + 8 * b, 1); mbar_init(b_empty_y + 8 * b, NW); }
@@ -283,7 +329,7 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
     if (lane == 0) {
       auto store_item = [&](long long m) {   // outputs of item m
         const int su = (int)(m % NUA);
-        const int iz0 = (int)((blockIdx.x + (m / nchunks) * gridDim.x) * TZ), c0 = (int)(m % nchunks) * VC;
+        const int iz0 = (int)(tile_of(blockIdx.x + (m / nchunks) * gridDim.x) * TZ), c0 = (int)(m % nchunks) * VC;
         mbar_wait_backoff(b_out_ready + 8 * su, (uint32_t)((m / NUA) & 1));
         const uint32_t src = s_ua + su * NARR * SM::PTILE;
         tma_store_3d(&tm_out, src, c0, iz0, 0);
@@ -291,11 +337,20 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
         tma_store_commit();
         tma_store_wait_read();   // the slot may be overwritten from here on
       };
-      long long tile = blockIdx.x;
+      long long ltile = blockIdx.x;
       int ch = 0;
       for (long long n = 0; n < nitems; ++n) {
+        const long long tile = tile_of(ltile);
         const int iz0 = (int)(tile * TZ);
         const int sy = (int)(n % NY);
+        if (ch == 0 && (p.wait_lo != nullptr || p.wait_hi != nullptr)) {
+          // z-slab: the ghost rows this tile reads (and the neighbour's ghost rows its edge rows overwrite) belong to
+          // the exchange with the neighbouring GPUs: wait for their rows of the previous stage
+          bool waited = false;
+          if (p.wait_lo != nullptr && tile * TZ < G) { wait_arrivals(p.wait_lo, p.wait_val, p.err_flag); waited = true; }
+          if (p.wait_hi != nullptr && (tile + 1) * TZ + G > p.nz) { wait_arrivals(p.wait_hi, p.wait_val, p.err_flag); waited = true; }
+          if (waited) asm volatile("fence.proxy.async.global;" ::: "memory");   // generic-proxy acquire -> TMA (async proxy) reads
+        }
         mbar_wait_backoff(b_empty_y + 8 * sy, (uint32_t)(((n / NY) & 1) ^ 1));
         mbar_expect_tx(b_full_y + 8 * sy, SM::YTILE);
         tma_load_3d(s_y + sy * SM::YTILE, &tm_y, b_full_y + 8 * sy, ch * VC, iz0 + G - H, 0);
@@ -314,7 +369,7 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
         } else {
           mbar_arrive(b_full_ua + 8 * su);   // nothing to load: the slot is free for staging
         }
-        if (++ch == nchunks) { ch = 0; tile += gridDim.x; }
+        if (++ch == nchunks) { ch = 0; ltile += gridDim.x; }
       }
       for (long long m = nitems > NUA ? nitems - NUA : 0; m < nitems; ++m) store_item(m);
       tma_store_wait_all();
@@ -329,22 +384,22 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
   for (int q = 0; q < 6 * S; ++q) msum[q] = 0.0;
   // lane l < 6S holds moment (l % 6) of row row0 + l / 6 of the stage input; the next tile's values are
   // fetched one tile ahead (and only touched at the next tile) so that their latency is never exposed
-  auto load_min = [&](long long t) {
+  auto load_min = [&](long long l) {   // l = position in the walk
     double m = 0.0;
-    if (lane < 6 * S && t < ntiles) {
-      const long long iz = t * TZ + row0 + lane / 6;
+    if (lane < 6 * S && l < ntiles) {
+      const long long iz = tile_of(l) * TZ + row0 + lane / 6;
       if (iz < p.nz) m = __ldg(p.mom_in + (long long)(lane % 6) * p.nz + iz);
     }
     return m;
   };
   double min_cur = 0.0, min_next = load_min(blockIdx.x);
-  long long tile = blockIdx.x;
+  long long ltile = blockIdx.x;
   int ch = 0;
   for (long long n = 0; n < nitems; ++n) {
-    const long long iz0 = tile * TZ;
+    const long long iz0 = tile_of(ltile) * TZ;
     if (ch == 0) {
       min_cur = p.mu * min_next;
-      min_next = load_min(tile + gridDim.x);
+      min_next = load_min(ltile + gridDim.x);
     }
     const int sy = (int)(n % NY), su = (int)(n % NUA);
     const uint32_t Ty = s_y + sy * SM::YTILE + lane * 8;                  // + ((c * ROWS + r) * 32) * 8
@@ -451,6 +506,13 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
           k[c] += cosenu_math::fd4_ko3(lds(b - 2 * VC * 8), lds(b - VC * 8), yc[c], lds(b + VC * 8), lds(b + 2 * VC * 8),
                                        cadv_v, p.cko);
         }
+      } else if constexpr (SCHEME == 2) {
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+          const uint32_t b = Ty + ((c * ROWS + tr) * VC) * 8;
+          k[c] += cosenu_math::fd4_ko5(lds(b - 3 * VC * 8), lds(b - 2 * VC * 8), lds(b - VC * 8), yc[c], lds(b + VC * 8),
+                                       lds(b + 2 * VC * 8), lds(b + 3 * VC * 8), cadv_v, p.cko);
+        }
       } else {
         if (s == 0) {
           double FL[8];
@@ -498,16 +560,18 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
         if constexpr (KT::WRITE_ACC) sts(Ta_out + cell, fma(p.ca, k[c], accb));
         out[c] = act ? o : 0.0;
       }
-      // periodic ghost rows of y_out (device rows outside 0..nz-1) are written directly
+      // ghost copies of the first / last G rows of y_out are written directly: my own periodic ghost rows, or the
+      // neighbouring slabs' ghost rows over NVLink (the halo exchange is fused into the producer)
       if (act && (iz < G || iz >= p.nz - G)) {
-        const long long gidx = (iz + G) * p.nvp + j;
         if (iz < G) {
+          double* d = p.ghost_lo_dst + iz * p.nvp + j;
 #pragma unroll
-          for (int c = 0; c < 8; ++c) p.y_out[c * p.comp_stride + gidx + p.nz * p.nvp] = out[c];
+          for (int c = 0; c < 8; ++c) d[c * p.ghost_lo_stride] = out[c];
         }
         if (iz >= p.nz - G) {
+          double* d = p.ghost_hi_dst + (iz - (p.nz - G)) * p.nvp + j;
 #pragma unroll
-          for (int c = 0; c < 8; ++c) p.y_out[c * p.comp_stride + gidx - p.nz * p.nvp] = out[c];
+          for (int c = 0; c < 8; ++c) d[c * p.ghost_hi_stride] = out[c];
         }
       }
 
@@ -543,8 +607,25 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
       }
 #pragma unroll
       for (int q = 0; q < 6 * S; ++q) msum[q] = 0.0;
+      // z-slab: tell the neighbours how many of their ghost rows this warp has just completed (all chunks)
+      if (p.sig_lo != nullptr || p.sig_hi != nullptr) {
+        int nlo = 0, nhi = 0;
+#pragma unroll
+        for (int s = 0; s < S; ++s) {
+          const long long iz = iz0 + row0 + s;
+          if (iz < p.nz) { nlo += iz < G; nhi += iz >= p.nz - G; }
+        }
+        if (nlo | nhi) {
+          __threadfence_system();   // every lane: its ghost stores before the signal
+          __syncwarp();
+          if (lane == 0) {
+            if (nlo && p.sig_lo != nullptr) red_add_release_sys(p.sig_lo, (unsigned long long)nlo);
+            if (nhi && p.sig_hi != nullptr) red_add_release_sys(p.sig_hi, (unsigned long long)nhi);
+          }
+        }
+      }
       ch = 0;
-      tile += gridDim.x;
+      ltile += gridDim.x;
     }
   }
 }

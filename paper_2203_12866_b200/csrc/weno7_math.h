@@ -141,5 +141,17 @@ COSENU_HD double fd4_ko3(double um2, double um1, double u0, double up1, double u
   return fma(-cadv, central, cko * fourth);
 }
 
+// FD4 + Kreiss-Oliger of order r = 3 (Eq. (5) PAPER.md:88-92 with r = 3: a 7-point operator): returns
+//   cadv * (u_{i-2} - 8u_{i-1} + 8u_{i+1} - u_{i+2}) + cko6 * (u_{i-3} - 6u_{i-2} + 15u_{i-1} - 20u_i + 15u_{i+1} - 6u_{i+2} + u_{i+3})
+// with cadv = -v/(12 dz), cko6 = +eps_ko/(64 dz): (D+ D-)^3 has the symbol -64 sin^6(k dz/2)/dz^6, so the dissipative
+// sign (reading A4) is PLUS the sixth difference.  On first differences, exactly 0 on z-uniform data.
+COSENU_HD double fd4_ko5(double um3, double um2, double um1, double u0, double up1, double up2, double up3, double cadv,
+                         double cko6) {
+  const double a = um2 - um3, b = um1 - um2, c = u0 - um1, d = up1 - u0, e = up2 - up1, f = up3 - up2;
+  const double central = fma(-7.0, c + d, b + e);
+  const double sixth = fma(10.0, d - c, fma(-5.0, e - b, f - a));
+  return fma(-cadv, central, cko6 * sixth);
+}
+
 }  // namespace cosenu_math
 #endif

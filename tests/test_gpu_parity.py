@@ -36,7 +36,7 @@ def run_pair(B, R, args, st, nsteps, **opts):
     gm = g.get_moments()
     gd = g.diagnostics()
     g.close()
-    ropts = {k: v for k, v in opts.items() if k in ("eps_ko", "weno_eps", "advect", "quadrature")}
+    ropts = {k: v for k, v in opts.items() if k in ("eps_ko", "weno_eps", "advect", "quadrature", "ko_order")}
     r = R.RefSim(*args, **ropts)
     r.set_state(st)
     r.step(nsteps)
@@ -173,6 +173,45 @@ def test_quadrature_option_rules(B):
     g.close()
 
 
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("nz,nv", [(64, 16), (77, 3), (250, 100), (5000, 33)])
+def test_ko_order_3(B, R, nz, nv, variant):
+    """FD4 + Kreiss-Oliger of order r = 3 (Eq. 5 with r = 3; halo 3): one rough step, then 20 steps of
+    the fast-conversion recipe, against the oracle; switching the order on a live handle re-encodes the boxes."""
+    st = inputs.random_state(nz, nv, seed=700 + nz + nv)
+    args = (nz, nv, 0.7 * nz, 0.05, 0.8, 0.3, 1.3, FD)
+    got, ref, gm, rm, _, _ = run_pair(B, R, args, st, 1, ko_order=3, eps_ko=0.3, variant=variant)
+    assert np.max(np.abs(got - ref)) <= 2e-14 * max(1.0, np.max(np.abs(ref)))
+    assert np.max(np.abs(gm - rm)) <= 1e-14 * max(1.0, np.max(np.abs(rm)))
+    st = inputs.fast_conversion_state(nz, nv, seed=42)
+    args = (nz, nv, float(nz), 0.4, 0.0, 0.0, 1.0, FD)
+    for rk_form in (0, 1, 2):
+        got, ref, *_ = run_pair(B, R, args, st, 20, ko_order=3, rk_form=rk_form, variant=variant)
+        assert np.max(np.abs(got - ref)) <= TOL20
+
+
+def test_ko_order_switch_on_live_handle(B, R):
+    nz, nv = 96, 12
+    st = inputs.random_state(nz, nv, seed=13)
+    args = (nz, nv, 96.0, 0.1, 0.0, 0.0, 0.7, FD)
+    g = B.Cosenu(*args)
+    g.set_state(st); g.step(2)                       # r = 2 boxes in use
+    g.set_option(B.OPT_KO_ORDER, 3)
+    g.set_state(st); g.step(2)
+    got = g.get_state()
+    g.set_option(B.OPT_KO_ORDER, 2)
+    g.set_state(st); g.step(2)
+    got2 = g.get_state()
+    g.close()
+    for ko, a in ((3, got), (2, got2)):
+        r = R.RefSim(*args, ko_order=ko)
+        r.set_state(st); r.step(2)
+        assert np.max(np.abs(a - r.get_state())) <= 1e-13, ko
+        r.close()
+    with pytest.raises(B.CosenuError):
+        B.Cosenu(*args).set_option(B.OPT_KO_ORDER, 4)
+
+
 def test_init_matches_oracle_init(B, R):
     """cosenu_init (library-side generator) gives bit-identical states to the oracle's and the input module's."""
     for kind in (0, 1, 2):
@@ -239,6 +278,39 @@ def test_library_owned_workspace(B, R):
     args = (nz, nv, 96.0, 0.1, 0.1, 0.2, 1.0, FD)
     got, ref, *_ = run_pair(B, R, args, st, 3, use_torch_workspace=False)
     assert np.max(np.abs(got - ref)) <= 1e-13
+
+
+@pytest.mark.parametrize("scheme", [FD, FV])
+def test_graph_replay_is_bitwise_identical(B, scheme):
+    """cosenu_step(n >= 16) replays a CUDA graph of 8 captured steps (COSENU_OPT_GRAPH): same launches, same results,
+    same bookkeeping as kernel-by-kernel launching; re-uploads and option changes keep it valid / rebuild it."""
+    nz, nv = 1024, 16
+    st = inputs.config_state("cfg0")
+    outs = []
+    for graph in (True, False):
+        g = B.Cosenu(nz, nv, float(nz), 0.4, 0.0, 0.0, 1.0, scheme, graph=graph)
+        g.set_state(st)
+        l0 = g.launch_count()
+        g.step(37)                       # 4 replays + 5 single steps
+        g.step(3)                        # below the threshold: direct
+        a = g.get_state()
+        d = g.diagnostics()
+        nl = g.launch_count() - l0
+        g.set_state(st)                  # the graph survives a re-upload (same buffers)
+        g.step(16)
+        b = g.get_state()
+        g.set_option(B.OPT_EPS_KO, 0.2)  # an option change drops it
+        g.set_option(B.OPT_WENO_EPS, 1e-5)
+        g.set_state(st)
+        g.step(16)
+        c = g.get_state()
+        outs.append((a, b, c, d["t"], d["step"], nl))
+        g.close()
+    for k in range(3):
+        assert np.array_equal(outs[0][k], outs[1][k]), k
+    assert outs[0][3] == outs[1][3] and outs[0][4] == outs[1][4] == 40
+    assert outs[0][5] == outs[1][5] == 4 * 40 + 1          # + the diagnostics kernel
+    assert not np.array_equal(outs[0][1], outs[0][2])       # the new options did take effect
 
 
 def test_bitwise_reproducible(B):

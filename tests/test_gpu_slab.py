@@ -1,0 +1,141 @@
+"""z-slab decomposition on ONE device: several slabs of one periodic grid, driven by one process on one
+stream (stage by stage, so that no kernel waits for a kernel queued behind it), against the single-domain solver and the
+oracle.  The decomposed path uses exactly the multi-GPU code: edge rows stored into the neighbouring slab's ghost rows,
+arrival counters, edge tiles first; only the peer mapping (same-process addresses instead of cudaIpcOpenMemHandle) differs.
+"""
+import numpy as np
+import pytest
+
+from paper_2203_12866_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+FD, FV = 0, 1
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2203_12866_b200 import binding
+    binding.load()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def S(B):
+    from paper_2203_12866_b200 import slab
+    return slab
+
+
+def _single(B, args, st, nsteps, **opts):
+    g = B.Cosenu(*args, **opts)
+    g.set_state(st)
+    g.step(nsteps)
+    out = g.get_state(), g.get_moments(), g.diagnostics()
+    g.close()
+    return out
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("scheme", [FD, FV])
+@pytest.mark.parametrize("nslabs,nz,nv", [(1, 200, 40), (2, 200, 40), (3, 200, 40), (2, 35, 5), (4, 5000, 33), (5, 16 * 5, 70)])
+def test_slab_group_equals_single_domain(B, S, scheme, nslabs, nz, nv, variant):
+    """Rough O(1) random state, 3 steps: the decomposed run reproduces the single-domain run bit for bit (same per-cell
+    arithmetic, same summation order of the moments), for ragged slabs, slabs of one tile, and a slab linked to itself."""
+    st = inputs.random_state(nz, nv, seed=500 + nz + nv)
+    args = (nz, nv, 0.7 * nz, 0.05, 0.8, 0.3, 1.3, scheme)
+    ref, refm, refd = _single(B, args, st, 3, variant=variant)
+    grp = S.SlabGroup(nslabs, *args, variant=variant)
+    grp.set_state(st)
+    grp.step(3)
+    grp.sync()
+    got, gotm, gotd = grp.get_state(), grp.get_moments(), grp.diagnostics()
+    grp.close()
+    assert np.array_equal(got, ref)
+    assert np.array_equal(gotm, refm)
+    for k in ("psurv_nu", "psurv_nubar", "dP_avg"):
+        assert abs(gotd[k] - refd[k]) <= 1e-13, k
+    for k in ("dP_max", "trace_dev_max", "ex_abs_max"):
+        assert abs(gotd[k] - refd[k]) <= 1e-13 * max(1.0, abs(refd[k])), k
+    assert np.max(np.abs(np.array(gotd["M0"]) - np.array(refd["M0"]))) <= 1e-12
+    assert gotd["step"] == 3 and abs(gotd["t"] - 0.15) < 1e-15
+
+
+@pytest.mark.parametrize("scheme", [FD, FV])
+@pytest.mark.parametrize("rk_form", [0, 1, 2])
+def test_slab_group_vs_oracle_20_steps(B, S, scheme, rk_form):
+    """BASELINE config 0 recipe over 3 uneven slabs, 20 steps, all RK carriers, against the oracle (1e-12)."""
+    from oracle import cosenu_ref as R
+    c = inputs.CONFIGS["cfg0"]
+    st = inputs.config_state("cfg0")
+    args = (c["nz"], c["nv"], c["L"], c["dt"], c["omega"], c["theta"], c["mu"], scheme)
+    grp = S.SlabGroup(3, *args, rk_form=rk_form, bounds=[(0, 100), (100, 600), (700, 324)])
+    grp.set_state(st)
+    grp.step(20)
+    grp.sync()
+    got = grp.get_state()
+    gd = grp.diagnostics()
+    grp.close()
+    r = R.RefSim(*args)
+    r.set_state(st)
+    r.step(20)
+    ref, rd = r.get_state(), r.diagnostics()
+    r.close()
+    assert np.max(np.abs(got - ref)) <= 1e-12
+    assert abs(gd["psurv_nu"] - rd["psurv_nu"]) <= 1e-12
+    assert max(abs(x) for x in gd["dM0"]) <= 1e-11
+
+
+def test_slab_init_builds_the_global_state(B, S):
+    """cosenu_init on slabs builds each slab's rows of the global seeded state (the splitmix64 stream is entered at
+    z_begin), for all three perturbation kinds."""
+    nz, nv = 700, 12
+    for kind in (0, 1, 2):
+        for scheme in (FD, FV):
+            args = (nz, nv, float(nz), 0.4, 0.0, 0.0, 1.0, scheme)
+            g = B.Cosenu(*args)
+            g.init(12866, pert_amp=1e-2 if kind == 2 else 1e-6, pert_kind=kind)
+            ref = g.get_state()
+            g.close()
+            grp = S.SlabGroup(3, *args)
+            grp.init(12866, pert_amp=1e-2 if kind == 2 else 1e-6, pert_kind=kind)
+            got = grp.get_state()
+            d = grp.diagnostics()
+            grp.close()
+            assert np.array_equal(got, ref), (kind, scheme)
+            assert abs(d["psurv_nu"] - 1.0) <= 1e-14
+
+
+def test_slab_self_linked_rank(B, S):
+    """CosenuSlab without torch.distributed = one slab linked to itself (the code path a 1-rank job takes)."""
+    nz, nv = 300, 20
+    st = inputs.fast_conversion_state(nz, nv, seed=11, pert_amp=1e-3)
+    args = (nz, nv, float(nz), 0.4, 1e-2, 0.01, 1.0, FV)
+    ref, refm, refd = _single(B, args, st, 10)
+    s = S.CosenuSlab(*args)
+    assert (s.world, s.rank, s.z_begin, s.nz) == (1, 0, 0, nz)
+    s.set_state(st)
+    s.step(10)
+    s.sync()
+    assert np.array_equal(s.get_state(), ref)
+    d = s.diagnostics()
+    assert abs(d["psurv_nu"] - refd["psurv_nu"]) <= 1e-13
+    s.close()
+
+
+def test_slab_call_order_errors(B, S):
+    h = B.Cosenu(64, 8, 64.0, 0.1, 0, 0, 1.0, FD, use_torch_workspace=False, slab=(128, 0))
+    h.set_state(inputs.random_state(64, 8, seed=1))
+    with pytest.raises(B.CosenuError) as e:
+        h.step(1)                                   # not linked, ghosts not exchanged
+    assert e.value.code == B.ESTATE
+    with pytest.raises(B.CosenuError) as e:
+        h.diagnostics()                             # a slab holds part of the grid
+    assert e.value.code == B.ESTATE
+    h.close()
+    with pytest.raises(B.CosenuError):
+        B.Cosenu(8, 8, 64.0, 0.1, 0, 0, 1.0, FD, slab=(128, 0))        # thinner than 16 rows
+    with pytest.raises(B.CosenuError):
+        B.Cosenu(64, 8, 64.0, 0.1, 0, 0, 1.0, FD, slab=(32, 0))        # larger than the grid

@@ -83,6 +83,19 @@ def test_kernel_fd_formula_matches_definition_and_is_exact_on_constants(libs):
         assert abs(a - b) <= 1e-14 / dz
     u = np.full(5, 0.7331)
     assert probe.cosenu_probe_fd4_ko3(u.ctypes.data_as(dp), 0.9, 1.0, 0.1) == 0.0
+    # Kreiss-Oliger r = 3 (Eq. 5): eps h^5 (D+ D-)^3 / 64 with the dissipative sign = + (eps/64dz) delta^6 u
+    probe.cosenu_probe_fd4_ko5.restype = C.c_double
+    probe.cosenu_probe_fd4_ko5.argtypes = [dp, C.c_double, C.c_double, C.c_double]
+    for _ in range(1000):
+        u = rng.standard_normal(7); v = rng.uniform(-1, 1); dz = rng.uniform(0.1, 2); ek = rng.uniform(0, 1)
+        a = probe.cosenu_probe_fd4_ko5(u.ctypes.data_as(dp), v, dz, ek)
+        d6 = u[0] - 6 * u[1] + 15 * u[2] - 20 * u[3] + 15 * u[4] - 6 * u[5] + u[6]
+        b = -v * (u[1] - 8 * u[2] + 8 * u[4] - u[5]) / (12 * dz) + (ek / (64 * dz)) * d6
+        assert abs(a - b) <= 2e-14 / dz
+    u = np.full(7, 0.7331)
+    assert probe.cosenu_probe_fd4_ko5(u.ctypes.data_as(dp), 0.9, 1.0, 0.1) == 0.0
+    u = (-1.0) ** np.arange(7)          # Nyquist mode: Q u = -(eps/dz) u at the centre cell (u_3 = -1)
+    assert abs(probe.cosenu_probe_fd4_ko5(u.ctypes.data_as(dp), 0.3, 1.0, 0.1) - 0.1) <= 1e-16
 
 
 def test_kernel_weno_form_against_exact_rational_algorithm1(libs):
