@@ -36,3 +36,55 @@ def test_cfg0_full_run_survival_probability(scheme):
     assert err <= 1e-9, err
     assert max(abs(x) for x in dg["dM0"]) <= 1e-10      # M0 conserved to rounding
     g.close(); r.close()
+
+
+def _read_series(path):
+    rows = []
+    with open(path) as f:
+        for line in f:
+            line = line.split("#", 1)[0].strip()
+            if line:
+                p = line.split()
+                rows.append((int(p[0]), float(p[1]), float(p[2]), float(p[3]), float(p[4])))
+    return rows
+
+
+# Step up to which the GPU run and the oracle agree to 1e-6 in the domain-averaged survival probability on BASELINE
+# config 2 (measured on B200, long runs).  Beyond it both runs are deep in the nonlinear regime,
+# where rounding-level differences between two correct fp64 evaluations are amplified at the instability's own rate.
+CFG2_AGREE_UNTIL = None    # None: the whole stored series
+
+
+def test_cfg2_long_run_against_stored_oracle_series():
+    """BASELINE config 2 (WENO7, 32768 x 128) against the oracle's stored time series
+    (tests/golden/cfg2_psurv_oracle.txt, written by tests/golden/make_longrun_psurv.py from oracle/ only)."""
+    import os
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "cfg2_psurv_oracle.txt")
+    if not os.path.exists(path):
+        pytest.skip("stored oracle series not present")
+    series = _read_series(path)
+    assert len(series) >= 10
+    from paper_2203_12866_b200 import binding as B
+    c = inputs.CONFIGS["cfg2"]
+    g = B.Cosenu(c["nz"], c["nv"], c["L"], c["dt"], c["omega"], c["theta"], c["mu"], c["scheme"])
+    g.set_state(inputs.config_state("cfg2"))
+    done, worst, first_bad, report = 0, 0.0, None, []
+    for step, ps_nu, ps_nubar, ex_max, dm0 in series:
+        g.step(step - done)
+        done = step
+        d = g.diagnostics()
+        err = max(abs(d["psurv_nu"] - ps_nu), abs(d["psurv_nubar"] - ps_nubar))
+        report.append((step, err, d["psurv_nu"]))
+        if CFG2_AGREE_UNTIL is None or step <= CFG2_AGREE_UNTIL:
+            worst = max(worst, err)
+        if err > 1e-6 and first_bad is None:
+            first_bad = step
+        assert max(abs(x) for x in d["dM0"]) <= 1e-9 * c["nz"]        # M0 conserved (PAPER.md:247-249), any length
+    g.close()
+    print("cfg2 long run: last step %d, worst |dPsurv| in the asserted range %.3e, first step above 1e-6: %s"
+          % (done, worst, first_bad))
+    print("  step, |dPsurv|, Psurv_gpu: " + "; ".join("%d %.2e %.6f" % r for r in report[::max(1, len(report) // 12)]))
+    assert worst <= 1e-6, (worst, first_bad)
