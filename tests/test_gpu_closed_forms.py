@@ -119,3 +119,38 @@ def test_conserved_quantity_scan_improves_with_resolution(B):
     assert rows[2]["dP_max"] < rows[1]["dP_max"] < rows[0]["dP_max"]
     assert all(r["dM0_max"] <= 1e-11 for r in rows)
     assert analysis.kappa(rows[0]["dP_avg"], rows[1]["dP_avg"], rows[2]["dP_avg"]) > 1.0
+
+
+@pytest.mark.parametrize("scheme", [FD, FV])
+def test_fiducial_run_respects_the_light_cone(B, scheme):
+    """The paper's fiducial fast-conversion run (alpha = 0.9, sigma = 0.6 / 0.5, Eq. (21) seed
+    eps(z) = 1e-2 exp(-z^2/50), N_z = 2000, N_v = 100, C_CFL = 0.2; the domain length is not printed -- 1200 here):
+    "flavor waves ... never cross the light cone" (|v| <= 1).  Inside the cone the instability has grown by orders of
+    magnitude; far outside it the off-diagonal elements are still at the level of the seed's Gaussian tail.  Also:
+    the beam v_z = 0.99 of Fig. 6 exists (bin centres), and M0 is conserved to rounding."""
+    nz, nv, L = 2000, 100, 1200.0
+    dz = L / nz
+    dt = 0.2 * dz
+    g = B.Cosenu(nz, nv, L, dt, 0.0, 0.0, 1.0, scheme)
+    g.init(1, pert_amp=1e-2, pert_kind=2)
+    st0 = g.get_state()
+    t_end = 250.0
+    nsteps = int(round(t_end / dt))
+    g.step(nsteps)
+    st = g.get_state()
+    d = g.diagnostics()
+    g.close()
+    assert abs(inputs.v_grid(nv)[-1] - 0.99) < 1e-15
+    zc = (np.arange(nz) + (0.5 if scheme == FV else 0.0)) * dz - 0.5 * L        # the seed is centred at L/2
+    gj = st0[0].max(axis=0)                                                      # g_nu(v) (rho_ee + rho_xx at t = 0)
+    ex = np.sqrt(st[2] ** 2 + st[3] ** 2) / gj[None, :]                          # |rho_ex| / g
+    inside = np.abs(zc) < 0.5 * t_end
+    outside = np.abs(zc) > t_end + 60.0                                          # light cone + the seed's own width
+    assert outside.sum() > 100
+    assert ex[inside].max() > 0.05                                               # the conversion has developed
+    assert ex[outside].max() < 1e-9                                              # and has not crossed the cone
+    assert max(abs(x) for x in d["dM0"]) <= 1e-10
+    assert d["trace_dev_max"] <= 1e-13
+    # waves propagate primarily toward +z (PAPER.md:267): more converted flavour on the +z side of the centre
+    pz = 1.0 - (st[0] / (st[0] + st[1]))                                         # rho_xx fraction per cell
+    assert pz[zc > 0].sum() > pz[zc < 0].sum()

@@ -626,3 +626,28 @@ def test_quadrature_option_validation():
         sim.set_option(R.OPT_QUADRATURE, 2)      # Simpson needs an odd number of points
     with pytest.raises(RuntimeError):
         sim.set_option(R.OPT_QUADRATURE, 3)
+
+
+# ----------------------------------------------------------------------------- causality of the fiducial run
+@pytest.mark.parametrize("scheme", [FD, FV])
+def test_fiducial_seed_stays_inside_the_light_cone(scheme):
+    """with the Eq. (21) seed "flavor waves are produced and propagate primarily toward the positive z
+    direction, but never cross the light cone".  |v| <= 1, so at time t nothing beyond |z - L/2| > t + (seed width) may
+    differ from the seed's Gaussian tail, while the centre has grown by orders of magnitude (the instability exists:
+    a wrong sign in the nu-nubar coupling or in the ELN crossing would leave the seed at 1e-2 / 2)."""
+    nz, nv, L = 500, 20, 300.0
+    dz = L / nz
+    dt = 0.2 * dz                                         # C_CFL = 0.2 (PAPER.md:267)
+    sim = R.RefSim(nz, nv, L, dt, 0.0, 0.0, 1.0, scheme)
+    sim.init(1, pert_amp=1e-2, pert_kind=2)
+    st0 = sim.get_state()
+    t_end = 70.0
+    sim.step(int(round(t_end / dt)))
+    st = sim.get_state()
+    zc = (np.arange(nz) + (0.5 if scheme == FV else 0.0)) * dz - 0.5 * L
+    gj = st0[0].max(axis=0)
+    ex = np.sqrt(st[2] ** 2 + st[3] ** 2) / gj[None, :]
+    assert ex[np.abs(zc) < 0.5 * t_end].max() > 0.02      # seed amplitude was 0.005: it has grown several-fold
+    assert ex[np.abs(zc) > t_end + 60.0].max() < 1e-12
+    pz = 1.0 - st[0] / (st[0] + st[1])
+    assert pz[zc > 0].sum() > pz[zc < 0].sum()            # forward-peaked angular distributions: waves go to +z
