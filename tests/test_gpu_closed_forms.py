@@ -150,7 +150,7 @@ def test_fiducial_run_respects_the_light_cone(B, scheme):
     assert ex[inside].max() > 0.05                                               # the conversion has developed
     assert ex[outside].max() < 1e-9                                              # and has not crossed the cone
     assert max(abs(x) for x in d["dM0"]) <= 1e-10
-    assert d["trace_dev_max"] <= 1e-13
+    assert d["trace_dev_max"] <= 1e-12                                           # 2083 steps of rounding on O(1) traces
     # waves propagate primarily toward +z: more converted flavour on the +z side of the centre
     pz = 1.0 - (st[0] / (st[0] + st[1]))                                         # rho_xx fraction per cell
     assert pz[zc > 0].sum() > pz[zc < 0].sum()
