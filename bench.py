@@ -36,12 +36,14 @@ UNIT = "cell-updates/s"
 # algorithmic HBM bytes per cell per stage launch:
 # read stage input + u0 + acc, write stage output + acc, 64 B each
 # per RK formulation (cosenu.h COSENU_OPT_RK_FORM): bytes per cell of stages 1..4
-STAGE_BYTES = {0: [192, 320, 320, 192], 1: [128, 256, 320, 192], 2: [128, 192, 192, 320]}
+STAGE_BYTES = {0: [192, 320, 320, 192], 1: [128, 256, 320, 192], 2: [128, 192, 192, 320], 3: [128, 256, 192, 192]}
 STAGE_KERNEL = {0: ["FIRST", "MID", "MID", "LAST"], 1: ["FIRST_LEAN", "MID_REBUILD", "MID", "LAST"],
-                2: ["FIRST_LEAN", "MID_NOACC", "MID_NOACC", "LAST_COMB"]}
-# dram__bytes_read.sum + dram__bytes_write.sum of the dominant stage launch (RK stage 4, LAST_COMB) from the
+                2: ["FIRST_LEAN", "MID_NOACC", "MID_NOACC", "LAST_COMB"],
+                3: ["FIRST_LEAN", "MID_P", "MID_NOACC", "LAST_P"]}
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant stage launch from the
 # committed ncu capture (profiles/r01_traffic_*.csv), per (workload, rk_form); None where not captured
-NCU_TRAFFIC_BYTES = {("cfg4", 2): 44279386880, ("cfg3", 2): 10752631296}   # profiles/r01_traffic_*.csv, RK stage 4
+NCU_TRAFFIC_BYTES = {("cfg4", 2): 44279386880, ("cfg3", 2): 10752631296,   # profiles/r01_traffic_*.csv, RK stage 4 (LAST_COMB)
+                     ("cfg4", 3): 34729661184, ("cfg3", 3): 8668317184}    # profiles/r01b_traffic_*.csv, RK stage 2 (MID_P)
 
 
 def measured_peaks():
@@ -324,7 +326,7 @@ def main():
     ap.add_argument("--workload", default="cfg4", choices=["cfg0", "cfg1", "cfg2", "cfg3", "cfg4"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
-    ap.add_argument("--rk-form", type=int, default=2, choices=[0, 1, 2])
+    ap.add_argument("--rk-form", type=int, default=3, choices=[0, 1, 2, 3])
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"])

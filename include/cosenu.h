@@ -57,7 +57,9 @@ enum {
                               0: accumulator array  ACC = u + dt/6 (k1 + 2k2 + 2k3), updated by every stage  (1024 B)
                               1: as 0, but stage 1 does not store ACC; stage 2 rebuilds k1 from (y2 - u) 2/dt  (896 B)
                               2: no accumulator: u+ = (y2 + 2 y3 + y4 - u)/3 + dt/6 k4 from the stage states   (832 B)
-                              default 2 */
+                              3: partial sum: stage 2, which holds u, y2 and y3, also stores P = (y2 + 2 y3 - u)/3;
+                                 stage 4 reads only P: u+ = P + y4/3 + dt/6 k4                                  (768 B)
+                              default 3 */
   COSENU_OPT_STAGE_TIMING = 4, /* 1: bracket every stage launch with CUDA events on the handle's stream
                               (read with cosenu_stage_times); default 0 */
   COSENU_OPT_VARIANT = 5,  /* kernel shape: 0 = 8 compute warps x 2 rows (default), 1 = 16 compute warps x 1 row;

@@ -41,7 +41,7 @@ struct cosenu {
   int64_t nz; int32_t nv; int nvp;
   double L, dt, omega, theta, mu; int scheme;
   double eps_ko = 0.1, weno_eps = 1e-6;
-  int advect = 1, rk_form = 2, stage_timing = 0;   // rk_form: 0 accumulator, 1 lean accumulator, 2 accumulator-free
+  int advect = 1, rk_form = 3, stage_timing = 0;   // rk_form: 0 accumulator, 1 lean accumulator, 2 accumulator-free, 3 partial sum
   int quad = 0;          // COSENU_OPT_QUADRATURE
   int ko_r = 2;          // COSENU_OPT_KO_ORDER: r of Eq. (5)
   double dz, dv, voff = 0.5;   // v_j = -1 + (j + voff) dv
@@ -228,6 +228,8 @@ int launch_kind(cosenu* h, int kind, const CUtensorMap& map, const CUtensorMap& 
     case MID_REBUILD: return launch_one<SCHEME, MID_REBUILD, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
     case LAST: return launch_one<SCHEME, LAST, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
     case MID_NOACC: return launch_one<SCHEME, MID_NOACC, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
+    case MID_P: return launch_one<SCHEME, MID_P, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
+    case LAST_P: return launch_one<SCHEME, LAST_P, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
     default: return launch_one<SCHEME, LAST_COMB, TZ, NSEG, NY, 1>(h, map, omap, a1, a2, p);   // 3 staged arrays: one slot
   }
 }
@@ -331,20 +333,20 @@ int rk_stage(cosenu* h, int k) {
     case 1:   // k2 = RHS(Y1); Y2 = U + dt/2 k2; [ACC += dt/3 k2]
       set_output(h, p, 2); p.acc_out = h->ACC; p.mom_in = Mout; p.mom_out = Min;
       p.cy = 0.5 * dt; p.ca = dt / 3.0;
-      rc = launch_stage(h, form == 0 ? MID : (form == 1 ? MID_REBUILD : MID_NOACC), h->tm_Y1, h->tp_Y2, h->tp_ACC,
-                        h->tp_ACC, p);
+      rc = launch_stage(h, form == 0 ? MID : (form == 1 ? MID_REBUILD : (form == 3 ? MID_P : MID_NOACC)), h->tm_Y1, h->tp_Y2,
+                        h->tp_ACC, h->tp_ACC, p);   // form 3: the "accumulator" written here is P = (Y2 + 2 Y3 - U)/3
       break;
     case 2:   // k3 = RHS(Y2); Y4 = U + dt k3 (into Y1, or into ACC in the accumulator-free form); [ACC += dt/3 k3]
       set_output(h, p, form == 2 ? 3 : 1); p.acc_out = h->ACC; p.mom_in = Min; p.mom_out = Mout;
       p.cy = dt; p.ca = dt / 3.0;
-      rc = launch_stage(h, form == 2 ? MID_NOACC : MID, h->tm_Y2, form == 2 ? h->tp_ACC : h->tp_Y1, h->tp_ACC,
-                        h->tp_ACC, p);
+      rc = launch_stage(h, (form == 2 || form == 3) ? MID_NOACC : MID, h->tm_Y2, form == 2 ? h->tp_ACC : h->tp_Y1,
+                        h->tp_ACC, h->tp_ACC, p);
       break;
     default:  // k4 = RHS(Y4); U = ACC + dt/6 k4   or   U = (Y2 + 2 Y3 + Y4 - U)/3 + dt/6 k4
       set_output(h, p, 0); p.acc_out = nullptr; p.mom_in = Mout; p.mom_out = Min;
       p.cy = dt / 6.0; p.ca = 0.0;
       if (form == 2) rc = launch_stage(h, LAST_COMB, h->tm_ACC, h->tp_U, h->tp_Y1, h->tp_Y2, p);
-      else rc = launch_stage(h, LAST, h->tm_Y1, h->tp_U, h->tp_ACC, h->tp_ACC, p);
+      else rc = launch_stage(h, form == 3 ? LAST_P : LAST, h->tm_Y1, h->tp_U, h->tp_ACC, h->tp_ACC, p);
       break;
   }
   if (rc == COSENU_OK && !h->dry_run) h->epoch++;
@@ -579,7 +581,7 @@ extern "C" int cosenu_set_option(cosenu_t* h, int key, double value) {
     case COSENU_OPT_EPS_KO: if (!(value >= 0) || !std::isfinite(value)) break; h->eps_ko = value; return COSENU_OK;
     case COSENU_OPT_WENO_EPS: if (!(value > 0) || !(value <= 1e30)) break; h->weno_eps = value; return COSENU_OK;
     case COSENU_OPT_ADVECT: h->advect = value != 0; return COSENU_OK;
-    case COSENU_OPT_RK_FORM: if (value != 0 && value != 1 && value != 2) break; h->rk_form = (int)value; return COSENU_OK;
+    case COSENU_OPT_RK_FORM: if (value != 0 && value != 1 && value != 2 && value != 3) break; h->rk_form = (int)value; return COSENU_OK;
     case COSENU_OPT_VARIANT: if (value != 0 && value != 1) break; h->variant = (int)value; return COSENU_OK;
     case COSENU_OPT_KO_ORDER:
       if (value != 2 && value != 3) break;

@@ -38,7 +38,10 @@ constexpr int VC = 32;  // beams per chunk = lanes of a warp
 //  lean accumulator  : FIRST_LEAN, MID_REBUILD, MID, LAST        896 B
 //  accumulator-free  : FIRST_LEAN, MID_NOACC, MID_NOACC, LAST_COMB   832 B:
 //      Y2 = U + dt/2 k1, Y3 = U + dt/2 k2, Y4 = U + dt k3,  U+ = (Y2 + 2 Y3 + Y4 - U)/3 + dt/6 k4
-enum StageKind { FIRST = 0, FIRST_LEAN = 1, MID = 2, MID_REBUILD = 3, LAST = 4, MID_NOACC = 5, LAST_COMB = 6 };
+//  partial sum       : FIRST_LEAN, MID_P, MID_NOACC, LAST_P            768 B:
+//      stage 2 also stores P = (Y2 + 2 Y3 - U)/3 (it holds all three); stage 4 reads only P: U+ = P + Y4/3 + dt/6 k4
+enum StageKind { FIRST = 0, FIRST_LEAN = 1, MID = 2, MID_REBUILD = 3, LAST = 4, MID_NOACC = 5, LAST_COMB = 6, MID_P = 7,
+                 LAST_P = 8 };
 
 struct StageParams {
   double* y_out;          // next stage input (FIRST/MID) or the new U (LAST)
@@ -155,10 +158,10 @@ __device__ __noinline__ void wait_arrivals(const unsigned long long* ctr, unsign
 
 template <int KIND>
 struct KindTraits {
-  static constexpr bool LOAD_U0 = (KIND == MID || KIND == MID_REBUILD || KIND == MID_NOACC || KIND == LAST_COMB);
-  static constexpr bool LOAD_ACC = (KIND == MID || KIND == LAST);
+  static constexpr bool LOAD_U0 = (KIND == MID || KIND == MID_REBUILD || KIND == MID_NOACC || KIND == LAST_COMB || KIND == MID_P);
+  static constexpr bool LOAD_ACC = (KIND == MID || KIND == LAST || KIND == LAST_P);
   static constexpr bool LOAD_Y23 = (KIND == LAST_COMB);   // the two earlier stage states Y2, Y3
-  static constexpr bool WRITE_ACC = (KIND == FIRST || KIND == MID || KIND == MID_REBUILD);
+  static constexpr bool WRITE_ACC = (KIND == FIRST || KIND == MID || KIND == MID_REBUILD || KIND == MID_P);
   static constexpr int NLOAD = (LOAD_U0 ? 1 : 0) + (LOAD_ACC ? 1 : 0) + (LOAD_Y23 ? 2 : 0);
   // staging arrays of one slot: array 0 = u0 on load (acc for LAST), y_out on store;
   //                             array 1 = acc on load (MID) / Y2 (LAST_COMB), acc_out on store; array 2 = Y3
@@ -547,17 +550,19 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
         const uint32_t cell = ((c * TZ + row) * VC) * 8;
         double u0v = yc[c], accb;
         if constexpr (KT::LOAD_U0) u0v = lds(Tu + cell);
-        if constexpr (KIND == FIRST || KIND == FIRST_LEAN || KIND == MID_NOACC) accb = yc[c];
+        if constexpr (KIND == FIRST || KIND == FIRST_LEAN || KIND == MID_NOACC || KIND == MID_P) accb = yc[c];
         else if constexpr (KIND == MID_REBUILD) accb = fma(yc[c] - u0v, 1.0 / 3.0, u0v);  // u0 + (dt/6) k1
         else if constexpr (KIND == LAST_COMB) {
           // (Y2 + 2 Y3 + Y4 - U) / 3 = U + dt/6 (k1 + 2 k2 + 2 k3); Y4 is the stage input itself
           const double y2 = lds(Tu + SM::PTILE + cell), y3 = lds(Tu + 2 * SM::PTILE + cell);
           accb = (fma(2.0, y3, y2) + (yc[c] - u0v)) * (1.0 / 3.0);
         } else accb = lds(Ta_in + cell);
-        const double base = (KIND == LAST || KIND == LAST_COMB) ? accb : u0v;
+        // LAST_P: accb = P = (Y2 + 2 Y3 - U)/3 and the stage input is Y4: U+ = P + Y4/3 + dt/6 k4
+        const double base = KIND == LAST_P ? fma(yc[c], 1.0 / 3.0, accb) : ((KIND == LAST || KIND == LAST_COMB) ? accb : u0v);
         const double o = fma(p.cy, k[c], base);
         sts(Tu + cell, o);
-        if constexpr (KT::WRITE_ACC) sts(Ta_out + cell, fma(p.ca, k[c], accb));
+        if constexpr (KIND == MID_P) sts(Ta_out + cell, (fma(2.0, o, yc[c]) - u0v) * (1.0 / 3.0));   // P; yc = Y2, o = Y3
+        else if constexpr (KT::WRITE_ACC) sts(Ta_out + cell, fma(p.ca, k[c], accb));
         out[c] = act ? o : 0.0;
       }
       // ghost copies of the first / last G rows of y_out are written directly: my own periodic ghost rows, or the
@@ -577,8 +582,8 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
 
       // ---- S5: velocity moments of the produced state, D = rho - rhobar^*
       {
-        const double dd = wq * ((out[0] - out[1]) - (out[4] - out[5])), dr = wq * (out[2] - out[6]),
-                     di = wq * (out[3] + out[7]);
+        double dd = (out[0] - out[1]) - (out[4] - out[5]), dr = out[2] - out[6], di = out[3] + out[7];
+        if (p.quad != 0) { dd *= wq; dr *= wq; di *= wq; }   // uniform branch: the default rule costs no fp64 issue slots
         msum[6 * s + 0] += dd;
         msum[6 * s + 1] = fma(v, dd, msum[6 * s + 1]);
         msum[6 * s + 2] += dr;

@@ -66,7 +66,7 @@ def test_one_step_random_state(B, R, scheme, nz, nv, variant):
 
 @pytest.mark.parametrize("variant", [0, 1])
 @pytest.mark.parametrize("scheme", [FD, FV])
-@pytest.mark.parametrize("lean", [0, 1, 2])
+@pytest.mark.parametrize("lean", [0, 1, 2, 3])
 def test_20_steps_cfg0_shape(B, R, scheme, lean, variant):
     """BASELINE config 0 (fast conversion, 1024 x 16, dt = 0.4 dz), 20 steps, both schemes."""
     c = inputs.CONFIGS["cfg0"]
@@ -185,7 +185,7 @@ def test_ko_order_3(B, R, nz, nv, variant):
     assert np.max(np.abs(gm - rm)) <= 1e-14 * max(1.0, np.max(np.abs(rm)))
     st = inputs.fast_conversion_state(nz, nv, seed=42)
     args = (nz, nv, float(nz), 0.4, 0.0, 0.0, 1.0, FD)
-    for rk_form in (0, 1, 2):
+    for rk_form in (0, 1, 2, 3):
         got, ref, *_ = run_pair(B, R, args, st, 20, ko_order=3, rk_form=rk_form, variant=variant)
         assert np.max(np.abs(got - ref)) <= TOL20
 

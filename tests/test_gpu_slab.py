@@ -64,7 +64,7 @@ def test_slab_group_equals_single_domain(B, S, scheme, nslabs, nz, nv, variant):
 
 
 @pytest.mark.parametrize("scheme", [FD, FV])
-@pytest.mark.parametrize("rk_form", [0, 1, 2])
+@pytest.mark.parametrize("rk_form", [0, 1, 2, 3])
 def test_slab_group_vs_oracle_20_steps(B, S, scheme, rk_form):
     """BASELINE config 0 recipe over 3 uneven slabs, 20 steps, all RK carriers, against the oracle (1e-12)."""
     from oracle import cosenu_ref as R
