@@ -220,6 +220,11 @@ int cosenu_slab_diag_finish(cosenu_t* h, const double* global10, int set_referen
  * waits for a kernel that is queued behind it). */
 int cosenu_slab_step_group(cosenu_t** hs, int32_t count, int64_t n);
 
+/* Enqueue ONE RK stage (k = 0..3, in this order; k = 3 completes the step) of a slab.  For drivers that put their own
+ * synchronisation between the stages, e.g. several processes sharing one GPU, where a kernel must never have to wait
+ * for a kernel of another process: sync + barrier after every stage, so every counter has arrived before the launch. */
+int cosenu_slab_stage(cosenu_t* h, int32_t k);
+
 /* 1 if a halo wait of this handle ever timed out (a neighbour did not arrive within ~4 s); synchronises. */
 int cosenu_slab_wait_failed(cosenu_t* h, int32_t* failed);
 

@@ -22,7 +22,7 @@ SYMBOLS = ["cosenu_create", "cosenu_workspace_bytes", "cosenu_attach", "cosenu_s
            "cosenu_sync", "cosenu_launch_count", "cosenu_stage_times", "cosenu_destroy", "cosenu_last_error",
            "cosenu_create_slab", "cosenu_slab_export", "cosenu_slab_link", "cosenu_slab_push_ghosts",
            "cosenu_slab_ref_sums", "cosenu_slab_set_ref_sums", "cosenu_slab_diag_sums", "cosenu_slab_diag_finish",
-           "cosenu_slab_step_group", "cosenu_slab_wait_failed"]
+           "cosenu_slab_step_group", "cosenu_slab_stage", "cosenu_slab_wait_failed"]
 
 
 class Diag(C.Structure):
@@ -89,6 +89,7 @@ def load():
     L.cosenu_slab_diag_sums.argtypes = [C.c_void_p, dp]
     L.cosenu_slab_diag_finish.argtypes = [C.c_void_p, dp, C.c_int, C.POINTER(Diag)]
     L.cosenu_slab_step_group.argtypes = [C.POINTER(C.c_void_p), C.c_int32, C.c_int64]
+    L.cosenu_slab_stage.argtypes = [C.c_void_p, C.c_int32]
     L.cosenu_slab_wait_failed.argtypes = [C.c_void_p, C.POINTER(C.c_int32)]
     _lib = L
     return L

@@ -913,6 +913,17 @@ extern "C" int cosenu_slab_step_group(cosenu_t** hs, int32_t count, int64_t n) {
   return COSENU_OK;
 }
 
+extern "C" int cosenu_slab_stage(cosenu_t* h, int32_t k) {
+  if (!h || k < 0 || k > 3) return h ? fail(h, COSENU_EINVAL, "cosenu_slab_stage: k must be 0..3") : COSENU_EINVAL;
+  if (!h->slab || !h->linked || !h->ghosts_pushed || !h->have_state)
+    return fail(h, COSENU_ESTATE, "cosenu_slab_stage: the slab must be linked, hold a state and have its ghosts exchanged");
+  CK(cudaSetDevice(h->device));
+  int rc = rk_stage(h, k);
+  if (rc) return rc;
+  if (k == 3) { h->t += h->dt; h->step += 1; }
+  return COSENU_OK;
+}
+
 extern "C" int cosenu_slab_wait_failed(cosenu_t* h, int32_t* failed) {
   if (!h || !failed) return COSENU_EINVAL;
   if (!h->maps_ready) { *failed = 0; return COSENU_OK; }

@@ -166,6 +166,16 @@ class CosenuSlab:
     def step(self, n=1):
         self.sim.step(n)
 
+    def step_lockstep(self, n=1):
+        """n steps with a device sync and a barrier over the ranks after EVERY stage: every arrival counter has reached its
+        value before the next launch, so no kernel ever waits for another process.  This is how ranks that share one GPU
+        must be driven (their kernels are time-sliced, not concurrent); with one GPU per rank use step()."""
+        for _ in range(int(n)):
+            for k in range(4):
+                self.sim._chk(self.sim._L.cosenu_slab_stage(self.sim.h, k))
+                self.sim.sync()
+                self.ring.barrier()
+
     def sync(self):
         self.sim.sync()
         if _wait_failed(self.sim):

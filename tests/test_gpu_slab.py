@@ -139,3 +139,60 @@ def test_slab_call_order_errors(B, S):
         B.Cosenu(8, 8, 64.0, 0.1, 0, 0, 1.0, FD, slab=(128, 0))        # thinner than 16 rows
     with pytest.raises(B.CosenuError):
         B.Cosenu(64, 8, 64.0, 0.1, 0, 0, 1.0, FD, slab=(32, 0))        # larger than the grid
+
+
+# ---------------------------------------------------------------------------------------------------------
+# The cross-PROCESS leg (cudaIpcGetMemHandle / cudaIpcOpenMemHandle, peer stores and counters in another process's
+# memory): two ranks share the one GPU, driven in lockstep (sync + barrier after every stage), so no kernel ever waits for
+# a kernel of the other process -- every counter has arrived before the launch that checks it.
+def _ipc_worker(rank, world, port, nz, nv, scheme, nsteps, q):
+    import os
+    import sys
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    import torch
+    import torch.distributed as dist
+    from paper_2203_12866_b200 import inputs as I, slab as S
+    torch.cuda.set_device(0)
+    import datetime
+    dist.init_process_group("gloo", rank=rank, world_size=world, timeout=datetime.timedelta(seconds=90))
+    try:
+        st = I.random_state(nz, nv, seed=900 + nz + nv)
+        s = S.CosenuSlab(nz, nv, 0.7 * nz, 0.05, 0.8, 0.3, 1.3, scheme)
+        s.set_state(np.ascontiguousarray(st[:, s.z_begin:s.z_begin + s.nz, :]))
+        s.step_lockstep(nsteps)
+        s.sync()
+        d = s.diagnostics()
+        q.put((rank, s.z_begin, s.nz, s.get_state(), d))
+        s.close()
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("scheme,world", [(FD, 2), (FV, 2), (FV, 3)])
+def test_slabs_in_separate_processes_over_cuda_ipc(B, scheme, world):
+    import torch.multiprocessing as mp
+    nz, nv, nsteps = 150, 40, 3
+    st = inputs.random_state(nz, nv, seed=900 + nz + nv)
+    args = (nz, nv, 0.7 * nz, 0.05, 0.8, 0.3, 1.3, scheme)
+    ref, _, refd = _single(B, args, st, nsteps)
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 29620 + 3 * scheme + world
+    ps = [ctx.Process(target=_ipc_worker, args=(r, world, port, nz, nv, scheme, nsteps, q)) for r in range(world)]
+    for p in ps:
+        p.start()
+    try:
+        outs = sorted((q.get(timeout=200) for _ in ps), key=lambda o: o[0])
+        for p in ps:
+            p.join(120)
+            assert p.exitcode == 0
+    finally:
+        for p in ps:
+            if p.is_alive():
+                p.terminate()
+    got = np.concatenate([o[3] for o in outs], axis=1)
+    assert [o[1] for o in outs][0] == 0 and sum(o[2] for o in outs) == nz
+    assert np.array_equal(got, ref)
+    for o in outs:
+        assert abs(o[4]["psurv_nu"] - refd["psurv_nu"]) <= 1e-13 and o[4]["step"] == nsteps
