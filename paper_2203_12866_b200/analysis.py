@@ -41,3 +41,17 @@ def conserved_quantity_scan(make_sim, nz_list, t_end, cfl=0.4, L=None, seed=1, p
                      "dM0_max": max(abs(x) for x in d["dM0"]), "psurv_nu": d["psurv_nu"]})
         sim.close()
     return rows
+
+
+def polarization_norm(state, species=0):
+    """|P|(z,v) of Eq. (4) from a canonical state (8, nz, nv): sqrt((ee-xx)^2 + 4 |ex|^2), un-normalised."""
+    o = 4 * species
+    st = np.asarray(state, dtype=np.float64)
+    return np.sqrt((st[o] - st[o + 1]) ** 2 + 4.0 * (st[o + 2] ** 2 + st[o + 3] ** 2))
+
+
+def dP_map(state, state0, species=0):
+    """The map delta P(z, v) = |P|(t) / |P|_0(v) - 1 of Fig. 10, |P|_0(v) = z-mean at t = 0 (the
+    reference cosenu_diagnostics uses for Eq. 22); its max |.| over (z,v) and both species is `dP_max`."""
+    p0 = polarization_norm(state0, species).mean(axis=0)
+    return polarization_norm(state, species) / p0[None, :] - 1.0

@@ -152,3 +152,19 @@ def test_kernel_weno_form_against_exact_rational_algorithm1(libs):
         assert abs(out[0] - a) <= 4e-16 * scale and abs(out[1] - b) <= 4e-16 * scale
     assert worst_kernel <= 2e-15, worst_kernel     # the kernels' form is accurate to a few ulp everywhere
     assert worst_oracle <= 5e-11, worst_oracle     # the literal form is right too, up to its cancellation noise
+
+
+def test_analysis_dP_map_matches_the_diagnostics_definition():
+    """analysis.dP_map (Fig. 10's delta P(z,v)) against Eq. (22) as the oracle's diagnostics take it."""
+    from oracle import cosenu_ref as R
+    from paper_2203_12866_b200 import analysis, inputs
+    c = inputs.CONFIGS["cfg0"]
+    st0 = inputs.config_state("cfg0")
+    r = R.RefSim(c["nz"], c["nv"], c["L"], c["dt"], 0.0, 0.0, 1.0, 0)
+    r.set_state(st0)
+    r.step(150)
+    d = r.diagnostics()
+    m = max(np.abs(analysis.dP_map(r.get_state(), st0, s)).max() for s in (0, 1))
+    assert abs(m - d["dP_max"]) <= 1e-13
+    assert analysis.dP_map(st0, st0).max() <= 1e-12      # 1e-6 seed: |P| is uniform in z to O(1e-12) at t = 0
+    r.close()
