@@ -217,19 +217,19 @@ int launch_one(cosenu* h, const CUtensorMap& map, const CUtensorMap& omap, const
   return COSENU_OK;
 }
 
-template <int SCHEME, int TZ, int NSEG, int NY, int NUA>
+template <int SCHEME, int TZ, int NSEG, int NY, int NUA, int NUA1 = NUA>   // NUA1: ring depth of the kinds that stage ONE array
 int launch_kind(cosenu* h, int kind, const CUtensorMap& map, const CUtensorMap& omap, const CUtensorMap& a1,
                 const CUtensorMap& a2, const StageParams& p) {
   switch (kind) {
     case FIRST: return launch_one<SCHEME, FIRST, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
     // stage 1 of the lean forms loads nothing but the stage input: a deeper input ring keeps enough bytes in flight
-    case FIRST_LEAN: return launch_one<SCHEME, FIRST_LEAN, TZ, NSEG, (SCHEME == 0 ? 4 : (SCHEME == 2 ? 3 : NY)), NUA>(h, map, omap, a1, a2, p);
+    case FIRST_LEAN: return launch_one<SCHEME, FIRST_LEAN, TZ, NSEG, (SCHEME == 0 ? 4 : (SCHEME == 2 ? 3 : NY)), NUA1>(h, map, omap, a1, a2, p);
     case MID: return launch_one<SCHEME, MID, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
     case MID_REBUILD: return launch_one<SCHEME, MID_REBUILD, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
-    case LAST: return launch_one<SCHEME, LAST, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
-    case MID_NOACC: return launch_one<SCHEME, MID_NOACC, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
+    case LAST: return launch_one<SCHEME, LAST, TZ, NSEG, NY, NUA1>(h, map, omap, a1, a2, p);
+    case MID_NOACC: return launch_one<SCHEME, MID_NOACC, TZ, NSEG, NY, NUA1>(h, map, omap, a1, a2, p);
     case MID_P: return launch_one<SCHEME, MID_P, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
-    case LAST_P: return launch_one<SCHEME, LAST_P, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
+    case LAST_P: return launch_one<SCHEME, LAST_P, TZ, NSEG, NY, NUA1>(h, map, omap, a1, a2, p);
     default: return launch_one<SCHEME, LAST_COMB, TZ, NSEG, NY, 1>(h, map, omap, a1, a2, p);   // 3 staged arrays: one slot
   }
 }
