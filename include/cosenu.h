@@ -62,8 +62,10 @@ enum {
                               default 3 */
   COSENU_OPT_STAGE_TIMING = 4, /* 1: bracket every stage launch with CUDA events on the handle's stream
                               (read with cosenu_stage_times); default 0 */
-  COSENU_OPT_VARIANT = 5,  /* kernel shape: 0 = 8 compute warps x 2 rows (default), 1 = 16 compute warps x 1 row;
-                              same arithmetic per cell, different summation grouping of the moments only */
+  COSENU_OPT_VARIANT = 5,  /* kernel shape: 0 = 8 compute warps x 2 rows per 16-row tile; WENO7 stages that stage one array use
+                              24-row tiles (3 rows per warp) when that does not quantise worse over the SMs (default);
+                              1 = 16 compute warps x 1 row; 2 = as 0 with the 24-row tiles forced; 3 = as 0 without them.
+                              Same arithmetic per cell in all shapes */
   COSENU_OPT_GRAPH = 8,    /* 1 (default): cosenu_step(n >= 16) replays a CUDA graph of 8 RK4 steps (32 kernel nodes) captured from the
                               handle's own launches, which removes the per-launch host cost on the small, launch-bound grids;
                               0: always launch kernel by kernel.  Not used on slab handles (their launch parameters change every

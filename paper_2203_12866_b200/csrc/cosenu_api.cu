@@ -29,6 +29,7 @@ typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_
 // tile shapes: TZ rows per tile, NSEG compute warps (S = TZ/NSEG rows each),
 // NY / NUA ring depths of the stage-input and of the u0/acc shared-memory slots.  `variant` picks a row.
 constexpr int TZ_ALL = 16;
+constexpr int TZ_WENO1 = 24;   // WENO7, kinds that stage one array: 3 rows per warp (shared differences, fewer boundary fluxes)
 constexpr int DIAG_BLOCKS = 592, DIAG_THREADS = 256, REF_BLOCKS = 148;
 
 std::string g_create_err;
@@ -57,8 +58,10 @@ struct cosenu {
   double *d_pref = nullptr, *d_p0ref = nullptr, *d_refpart = nullptr, *d_diagpart = nullptr;
   int64_t comp_stride = 0; size_t state_elems = 0;
   int mcur = 0;  // M[mcur] holds the moments of U
-  CUtensorMap tm_U, tm_Y1, tm_Y2, tm_ACC;   // stage-input boxes [8][TZ+2H][32]
-  CUtensorMap tp_U, tp_Y1, tp_Y2, tp_ACC;   // rows 0..nz-1 only, boxes [8][TZ][32]: u0 / acc loads, output stores
+  // tensor maps per tile height (index 0: TZ = 16, 1: TZ = 24 [WENO7 kinds that stage one array]) and per state buffer
+  // (0 U, 1 Y1, 2 Y2, 3 ACC)
+  CUtensorMap tm[2][4];   // stage-input boxes [8][TZ+2H][32] over the ghosted rows
+  CUtensorMap tp[2][4];   // rows 0..nz-1 only, boxes [8][TZ][32]: u0 / acc loads, output stores
   bool maps_ready = false;
 
   bool have_state = false;
@@ -183,22 +186,22 @@ int make_maps(cosenu* h) {
   CK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr));
   if (!fn || qr != cudaDriverEntryPointSuccess) return fail(h, COSENU_ECUDA, "cuTensorMapEncodeTiled not available in this driver");
   PFN_encodeTiled enc = reinterpret_cast<PFN_encodeTiled>(fn);
-  const int rows = TZ_ALL + 2 * (h->scheme == COSENU_FD4_KO3 ? h->ko_r : 4);
-  int rc;
-  if ((rc = make_map(h, enc, &h->tm_U, h->U, rows, true))) return rc;
-  if ((rc = make_map(h, enc, &h->tm_Y1, h->Y1, rows, true))) return rc;
-  if ((rc = make_map(h, enc, &h->tm_Y2, h->Y2, rows, true))) return rc;
-  if ((rc = make_map(h, enc, &h->tm_ACC, h->ACC, rows, true))) return rc;
-  if ((rc = make_map(h, enc, &h->tp_U, h->U, TZ_ALL, false))) return rc;
-  if ((rc = make_map(h, enc, &h->tp_Y1, h->Y1, TZ_ALL, false))) return rc;
-  if ((rc = make_map(h, enc, &h->tp_Y2, h->Y2, TZ_ALL, false))) return rc;
-  if ((rc = make_map(h, enc, &h->tp_ACC, h->ACC, TZ_ALL, false))) return rc;
+  const int halo = h->scheme == COSENU_FD4_KO3 ? h->ko_r : 4;
+  double* bufs[4] = {h->U, h->Y1, h->Y2, h->ACC};
+  const int tzs[2] = {TZ_ALL, TZ_WENO1};
+  for (int t = 0; t < (h->scheme == COSENU_FV_WENO7 ? 2 : 1); ++t)
+    for (int b = 0; b < 4; ++b) {
+      int rc;
+      if ((rc = make_map(h, enc, &h->tm[t][b], bufs[b], tzs[t] + 2 * halo, true))) return rc;
+      if ((rc = make_map(h, enc, &h->tp[t][b], bufs[b], tzs[t], false))) return rc;
+    }
   return COSENU_OK;
 }
 
 template <int SCHEME, int KIND, int TZ, int NSEG, int NY, int NUA>
-int launch_one(cosenu* h, const CUtensorMap& map, const CUtensorMap& omap, const CUtensorMap& a1, const CUtensorMap& a2,
-               const StageParams& p) {
+int launch_one(cosenu* h, int in_buf, int out_buf, int a1_buf, int a2_buf, const StageParams& p0) {
+  constexpr int T = TZ == TZ_ALL ? 0 : 1;
+  const CUtensorMap &map = h->tm[T][in_buf], &omap = h->tp[T][out_buf], &a1 = h->tp[T][a1_buf], &a2 = h->tp[T][a2_buf];
   auto kern = stage_kernel<SCHEME, KIND, TZ, NSEG, NY, NUA>;
   constexpr size_t smem = StageSmem<SCHEME, KIND, TZ, NSEG, NY, NUA>::bytes;
   static_assert(smem <= 232448, "over the 227 KB shared-memory limit of a CTA");
@@ -211,31 +214,39 @@ int launch_one(cosenu* h, const CUtensorMap& map, const CUtensorMap& omap, const
   if (h->dry_run) return COSENU_OK;
   const long long ntiles = (h->nz + TZ - 1) / TZ;
   const unsigned grid = (unsigned)(ntiles < h->num_sms ? ntiles : h->num_sms);   // persistent: one CTA per SM
-  kern<<<grid, NSEG * 32 + 32, smem, h->stream>>>(map, h->tp_U, a1, a2, omap, p);
+  StageParams p = p0;
+  if (h->slab) p.tile_shift = ntiles >= 3 ? ntiles - 2 : 0;   // walk the (up to two) high edge tiles, then tile 0, first
+  kern<<<grid, NSEG * 32 + 32, smem, h->stream>>>(map, h->tp[T][0], a1, a2, omap, p);
   CK(cudaGetLastError());
   h->launches++;
   return COSENU_OK;
 }
 
 template <int SCHEME, int TZ, int NSEG, int NY, int NUA, int NUA1 = NUA>   // NUA1: ring depth of the kinds that stage ONE array
-int launch_kind(cosenu* h, int kind, const CUtensorMap& map, const CUtensorMap& omap, const CUtensorMap& a1,
-                const CUtensorMap& a2, const StageParams& p) {
+int launch_kind(cosenu* h, int kind, int map, int omap, int a1, int a2, const StageParams& p) {
+  // kinds that stage ONE array (they also fit tiles of TZ_WENO1 rows)
   switch (kind) {
-    case FIRST: return launch_one<SCHEME, FIRST, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
     // stage 1 of the lean forms loads nothing but the stage input: a deeper input ring keeps enough bytes in flight
     case FIRST_LEAN: return launch_one<SCHEME, FIRST_LEAN, TZ, NSEG, (SCHEME == 0 ? 4 : (SCHEME == 2 ? 3 : NY)), NUA1>(h, map, omap, a1, a2, p);
-    case MID: return launch_one<SCHEME, MID, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
-    case MID_REBUILD: return launch_one<SCHEME, MID_REBUILD, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
     case LAST: return launch_one<SCHEME, LAST, TZ, NSEG, NY, NUA1>(h, map, omap, a1, a2, p);
     case MID_NOACC: return launch_one<SCHEME, MID_NOACC, TZ, NSEG, NY, NUA1>(h, map, omap, a1, a2, p);
-    case MID_P: return launch_one<SCHEME, MID_P, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
     case LAST_P: return launch_one<SCHEME, LAST_P, TZ, NSEG, NY, NUA1>(h, map, omap, a1, a2, p);
-    default: return launch_one<SCHEME, LAST_COMB, TZ, NSEG, NY, 1>(h, map, omap, a1, a2, p);   // 3 staged arrays: one slot
+    default: break;
   }
+  if constexpr (TZ == TZ_ALL) {   // two or three staged arrays
+    switch (kind) {
+      case FIRST: return launch_one<SCHEME, FIRST, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
+      case MID: return launch_one<SCHEME, MID, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
+      case MID_REBUILD: return launch_one<SCHEME, MID_REBUILD, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
+      case MID_P: return launch_one<SCHEME, MID_P, TZ, NSEG, NY, NUA>(h, map, omap, a1, a2, p);
+      case LAST_COMB: return launch_one<SCHEME, LAST_COMB, TZ, NSEG, NY, 1>(h, map, omap, a1, a2, p);   // 3 staged arrays: one slot
+      default: break;
+    }
+  }
+  return fail(h, COSENU_EINVAL, "launch_kind: no kernel for this stage kind and tile height");
 }
 
-int launch_stage(cosenu* h, int kind, const CUtensorMap& map, const CUtensorMap& omap, const CUtensorMap& a1,
-                 const CUtensorMap& a2, const StageParams& p) {
+int launch_stage(cosenu* h, int kind, int map, int omap, int a1, int a2, const StageParams& p) {
   if (h->scheme == COSENU_FD4_KO3 && h->ko_r == 3) {   // FD4 + Kreiss-Oliger r = 3: halo 3
     if (h->variant == 1) return launch_kind<2, TZ_ALL, 16, 2, 2>(h, kind, map, omap, a1, a2, p);
     return launch_kind<2, TZ_ALL, 8, 2, 2>(h, kind, map, omap, a1, a2, p);
@@ -245,6 +256,15 @@ int launch_stage(cosenu* h, int kind, const CUtensorMap& map, const CUtensorMap&
     return launch_kind<0, TZ_ALL, 8, 2, 2>(h, kind, map, omap, a1, a2, p);
   }
   if (h->variant == 1) return launch_kind<1, TZ_ALL, 16, 2, 1>(h, kind, map, omap, a1, a2, p);
+  // the kinds that stage one array leave room for tiles of 24 rows = 3 rows per warp: the undivided differences are
+  // shared by three interfaces and the tile-boundary flux is recomputed once per 24 rows instead of 16
+  // ... unless the coarser tiles quantise worse over the persistent grid (rows walked by the busiest CTA; the taller
+  // tile is worth about 2 %): e.g. nz = 32768 is 13.8 waves of 16-row tiles but 9.2 waves of 24-row tiles
+  const long long w16 = ((h->nz + TZ_ALL - 1) / TZ_ALL + h->num_sms - 1) / h->num_sms * TZ_ALL;
+  const long long w24 = ((h->nz + TZ_WENO1 - 1) / TZ_WENO1 + h->num_sms - 1) / h->num_sms * TZ_WENO1;
+  const bool tz24 = h->variant == 2 || (h->variant == 0 && 0.98 * (double)w24 <= (double)w16);   // variant 3: never
+  if (tz24 && (kind == FIRST_LEAN || kind == MID_NOACC || kind == LAST_P || kind == LAST))
+    return launch_kind<1, TZ_WENO1, 8, 2, 1>(h, kind, map, omap, a1, a2, p);
   return launch_kind<1, TZ_ALL, 8, 2, 1>(h, kind, map, omap, a1, a2, p);
 }
 
@@ -310,8 +330,6 @@ void set_output(cosenu* h, StageParams& p, int which) {
   p.wait_hi = h->d_ctr + 1;
   p.wait_val = (unsigned long long)G * h->epoch;   // G rows per edge per stage launch so far
   p.err_flag = h->d_err;
-  const long long ntiles = (h->nz + TZ_ALL - 1) / TZ_ALL;
-  p.tile_shift = ntiles >= 3 ? ntiles - 2 : 0;     // walk the (up to two) high edge tiles, then tile 0, first
 }
 
 // RK stage k (0..3) of the classical RK4 step = ONE fused launch.  Buffers: U -> Y1 -> Y2 -> (Y1 | ACC) -> U; in the
@@ -328,25 +346,23 @@ int rk_stage(cosenu* h, int k) {
     case 0:   // k1 = RHS(U); Y1 = U + dt/2 k1; [ACC = U + dt/6 k1]
       set_output(h, p, 1); p.acc_out = h->ACC; p.mom_in = Min; p.mom_out = Mout;
       p.cy = 0.5 * dt; p.ca = dt / 6.0;
-      rc = launch_stage(h, form == 0 ? FIRST : FIRST_LEAN, h->tm_U, h->tp_Y1, h->tp_ACC, h->tp_ACC, p);
+      rc = launch_stage(h, form == 0 ? FIRST : FIRST_LEAN, 0, 1, 3, 3, p);
       break;
     case 1:   // k2 = RHS(Y1); Y2 = U + dt/2 k2; [ACC += dt/3 k2]
       set_output(h, p, 2); p.acc_out = h->ACC; p.mom_in = Mout; p.mom_out = Min;
       p.cy = 0.5 * dt; p.ca = dt / 3.0;
-      rc = launch_stage(h, form == 0 ? MID : (form == 1 ? MID_REBUILD : (form == 3 ? MID_P : MID_NOACC)), h->tm_Y1, h->tp_Y2,
-                        h->tp_ACC, h->tp_ACC, p);   // form 3: the "accumulator" written here is P = (Y2 + 2 Y3 - U)/3
+      rc = launch_stage(h, form == 0 ? MID : (form == 1 ? MID_REBUILD : (form == 3 ? MID_P : MID_NOACC)), 1, 2, 3, 3, p);   // form 3: the "accumulator" written here is P = (Y2 + 2 Y3 - U)/3
       break;
     case 2:   // k3 = RHS(Y2); Y4 = U + dt k3 (into Y1, or into ACC in the accumulator-free form); [ACC += dt/3 k3]
       set_output(h, p, form == 2 ? 3 : 1); p.acc_out = h->ACC; p.mom_in = Min; p.mom_out = Mout;
       p.cy = dt; p.ca = dt / 3.0;
-      rc = launch_stage(h, (form == 2 || form == 3) ? MID_NOACC : MID, h->tm_Y2, form == 2 ? h->tp_ACC : h->tp_Y1,
-                        h->tp_ACC, h->tp_ACC, p);
+      rc = launch_stage(h, (form == 2 || form == 3) ? MID_NOACC : MID, 2, form == 2 ? 3 : 1, 3, 3, p);
       break;
     default:  // k4 = RHS(Y4); U = ACC + dt/6 k4   or   U = (Y2 + 2 Y3 + Y4 - U)/3 + dt/6 k4
       set_output(h, p, 0); p.acc_out = nullptr; p.mom_in = Mout; p.mom_out = Min;
       p.cy = dt / 6.0; p.ca = 0.0;
-      if (form == 2) rc = launch_stage(h, LAST_COMB, h->tm_ACC, h->tp_U, h->tp_Y1, h->tp_Y2, p);
-      else rc = launch_stage(h, form == 3 ? LAST_P : LAST, h->tm_Y1, h->tp_U, h->tp_ACC, h->tp_ACC, p);
+      if (form == 2) rc = launch_stage(h, LAST_COMB, 3, 0, 1, 2, p);
+      else rc = launch_stage(h, form == 3 ? LAST_P : LAST, 1, 0, 3, 3, p);
       break;
   }
   if (rc == COSENU_OK && !h->dry_run) h->epoch++;
@@ -582,7 +598,7 @@ extern "C" int cosenu_set_option(cosenu_t* h, int key, double value) {
     case COSENU_OPT_WENO_EPS: if (!(value > 0) || !(value <= 1e30)) break; h->weno_eps = value; return COSENU_OK;
     case COSENU_OPT_ADVECT: h->advect = value != 0; return COSENU_OK;
     case COSENU_OPT_RK_FORM: if (value != 0 && value != 1 && value != 2 && value != 3) break; h->rk_form = (int)value; return COSENU_OK;
-    case COSENU_OPT_VARIANT: if (value != 0 && value != 1) break; h->variant = (int)value; return COSENU_OK;
+    case COSENU_OPT_VARIANT: if (value != 0 && value != 1 && value != 2 && value != 3) break; h->variant = (int)value; return COSENU_OK;
     case COSENU_OPT_KO_ORDER:
       if (value != 2 && value != 3) break;
       if (h->ko_r != (int)value) {

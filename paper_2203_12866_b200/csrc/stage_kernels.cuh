@@ -234,7 +234,7 @@ __device__ __forceinline__ void butterfly_reduce(double (&x)[N], int lane, int& 
 // FR[s][c] = WENO7 value of u_c at the right interface of row (rel_row + s).
 template <int DIR, int S, int ROWS, int H>
 __device__ __forceinline__ void weno_rows(uint32_t Tw, const cosenu_math::Weno7Beam& bm, double (&FR)[S][8]) {
-  static_assert(S == 1 || S == 2, "rows per warp");
+  static_assert(S == 1 || S == 2 || S == 3, "rows per warp");
 #pragma unroll
   for (int c = 0; c < 8; ++c) {
     if constexpr (S == 1) {
@@ -242,13 +242,22 @@ __device__ __forceinline__ void weno_rows(uint32_t Tw, const cosenu_math::Weno7B
 #pragma unroll
       for (int k = 0; k < 7; ++k) w[k] = lds(Tw + ((c * ROWS + H + (DIR > 0 ? 0 : 1) + DIR * (k - 3)) * VC) * 8);
       FR[0][c] = cosenu_math::weno7_face(w, bm);
-    } else {
+    } else if constexpr (S == 2) {
       double w[8], Fa, Fb;
 #pragma unroll
       for (int k = 0; k < 8; ++k) w[k] = lds(Tw + ((c * ROWS + H + (DIR > 0 ? k - 3 : 5 - k)) * VC) * 8);
       cosenu_math::weno7_face2(w, bm, Fa, Fb);
       FR[DIR > 0 ? 0 : 1][c] = Fa;
       FR[DIR > 0 ? 1 : 0][c] = Fb;
+    } else {
+      // three rows per warp: 9 cells, the undivided differences are shared by the three interfaces
+      double w[9], Fa, Fb, Fc;
+#pragma unroll
+      for (int k = 0; k < 9; ++k) w[k] = lds(Tw + ((c * ROWS + H + (DIR > 0 ? k - 3 : 6 - k)) * VC) * 8);
+      cosenu_math::weno7_face3(w, bm, Fa, Fb, Fc);
+      FR[DIR > 0 ? 0 : 2][c] = Fa;
+      FR[1][c] = Fb;
+      FR[DIR > 0 ? 2 : 0][c] = Fc;
     }
   }
 }

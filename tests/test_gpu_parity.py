@@ -52,7 +52,7 @@ def run_pair(B, R, args, st, nsteps, **opts):
 SHAPES = [(64, 16), (1024, 16), (100, 8), (77, 3), (96, 40), (250, 100), (129, 130), (16, 2), (5000, 33)]
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 @pytest.mark.parametrize("scheme", [FD, FV])
 @pytest.mark.parametrize("nz,nv", SHAPES)
 def test_one_step_random_state(B, R, scheme, nz, nv, variant):
@@ -64,7 +64,7 @@ def test_one_step_random_state(B, R, scheme, nz, nv, variant):
     assert np.max(np.abs(gm - rm)) <= 1e-14 * max(1.0, np.max(np.abs(rm)))
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 @pytest.mark.parametrize("scheme", [FD, FV])
 @pytest.mark.parametrize("lean", [0, 1, 2, 3])
 def test_20_steps_cfg0_shape(B, R, scheme, lean, variant):

@@ -38,7 +38,7 @@ def _single(B, args, st, nsteps, **opts):
     return out
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 @pytest.mark.parametrize("scheme", [FD, FV])
 @pytest.mark.parametrize("nslabs,nz,nv", [(1, 200, 40), (2, 200, 40), (3, 200, 40), (2, 35, 5), (4, 5000, 33), (5, 16 * 5, 70)])
 def test_slab_group_equals_single_domain(B, S, scheme, nslabs, nz, nv, variant):
