@@ -43,7 +43,7 @@ STAGE_KERNEL = {0: ["FIRST", "MID", "MID", "LAST"], 1: ["FIRST_LEAN", "MID_REBUI
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant stage launch from the
 # committed ncu capture (profiles/r01_traffic_*.csv), per (workload, rk_form); None where not captured
 NCU_TRAFFIC_BYTES = {("cfg4", 2): 44279386880, ("cfg3", 2): 10752631296,   # profiles/r01_traffic_*.csv, RK stage 4 (LAST_COMB)
-                     ("cfg4", 3): 34729661184, ("cfg3", 3): 8668317184}    # profiles/r01b_traffic_*.csv, RK stage 2 (MID_P)
+                     ("cfg4", 3): 34764352512, ("cfg3", 3): 8683646720}    # profiles/r01b_traffic_*.csv, RK stage 2 (MID_P)
 
 
 def measured_peaks():
