@@ -46,6 +46,14 @@ NCU_TRAFFIC_BYTES = {("cfg4", 2): 44279386880, ("cfg3", 2): 10752631296,   # pro
                      ("cfg4", 3): 34764352512, ("cfg3", 3): 8683646720}    # profiles/r01b_traffic_*.csv, RK stage 2 (MID_P)
 
 
+# fp64 instructions (DFMA + DMUL + DADD, per thread = per (z,v) cell) one stage launch executes per cell, from
+# smsp__sass_thread_inst_executed_op_d{fma,mul,add}_pred_on.sum of the committed capture (profiles/r01b_fp64_*.csv): the
+# ALU side of the roofline.  Peak = 148 SMs x 4 sub-partitions x 16 fp64 lanes per clock x 1.965 GHz.
+FP64_PER_CELL = {"WENO7": {"FIRST_LEAN": None, "MID_P": None, "MID_NOACC": None, "LAST_P": None},
+                 "FD4_KO3": {"FIRST_LEAN": None, "MID_P": None, "MID_NOACC": None, "LAST_P": None}}
+FP64_PEAK_LANE_OPS = 148 * 4 * 16 * 1.965e9
+
+
 def measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -294,6 +302,15 @@ def run_ours(args):
                   "GBps": sb[k] * cells / (avg[k] * 1e-3) / 1e9} for k in range(4)] if nst else []
     dom = max(range(4), key=lambda k: avg[k]) if nst else 0
     achieved = per_stage[dom]["GBps"] if nst else None
+    # the same launch against the plain fp64 ALU peak (WENO7 is co-bound by it; FD is not)
+    sname = "WENO7" if c["scheme"] else "FD4_KO3"
+    nfp = FP64_PER_CELL[sname].get(STAGE_KERNEL[args.rk_form][dom]) if nst else None
+    alu = None
+    if nfp:
+        a = nfp * cells / (avg[dom] * 1e-3)
+        alu = {"achieved": a / 1e12, "peak": FP64_PEAK_LANE_OPS / 1e12, "unit": "T fp64 instr/s (per lane; x2 for FMA flops)",
+               "frac": a / FP64_PEAK_LANE_OPS, "fp64_instr_per_cell_launch": nfp,
+               "peak_source": "148 SMs x 4 SMSPs x 16 lanes/clk x 1.965 GHz (max SM clock; sustained clock is lower under sw_power_cap)"}
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak if achieved else None,
                 "traffic": NCU_TRAFFIC_BYTES.get((c["name"], args.rk_form)), "peak_source": peak_src,
@@ -301,7 +318,7 @@ def run_ours(args):
                                                                   STAGE_KERNEL[args.rk_form][dom], dom + 1),
                 "algorithmic_bytes_per_launch": sb[dom] * cells, "avg_launch_ms": avg[dom],
                 "stage_kernel_share_of_step": sum(avg) / (ms / args.steps) if nst else None,
-                "per_stage": per_stage, "bytes_per_cell_step": step_bytes,
+                "alu": alu, "per_stage": per_stage, "bytes_per_cell_step": step_bytes,
                 "step_model_GBps": step_bytes * value / world / 1e9,
                 "step_model_frac": step_bytes * value / world / 1e9 / peak,
                 # "effective" bandwidth with the fused 3-array traffic model (1024 B per cell-step),

@@ -189,12 +189,14 @@ int make_maps(cosenu* h) {
   const int halo = h->scheme == COSENU_FD4_KO3 ? h->ko_r : 4;
   double* bufs[4] = {h->U, h->Y1, h->Y2, h->ACC};
   const int tzs[2] = {TZ_ALL, TZ_WENO1};
-  for (int t = 0; t < (h->scheme == COSENU_FV_WENO7 ? 2 : 1); ++t)
+  for (int t = 0; t < 2; ++t) {
+    if (t == 1 && h->scheme != COSENU_FV_WENO7) continue;
     for (int b = 0; b < 4; ++b) {
       int rc;
       if ((rc = make_map(h, enc, &h->tm[t][b], bufs[b], tzs[t] + 2 * halo, true))) return rc;
       if ((rc = make_map(h, enc, &h->tp[t][b], bufs[b], tzs[t], false))) return rc;
     }
+  }
   return COSENU_OK;
 }
 
@@ -226,8 +228,9 @@ template <int SCHEME, int TZ, int NSEG, int NY, int NUA, int NUA1 = NUA>   // NU
 int launch_kind(cosenu* h, int kind, int map, int omap, int a1, int a2, const StageParams& p) {
   // kinds that stage ONE array (they also fit tiles of TZ_WENO1 rows)
   switch (kind) {
-    // stage 1 of the lean forms loads nothing but the stage input: a deeper input ring keeps enough bytes in flight
-    case FIRST_LEAN: return launch_one<SCHEME, FIRST_LEAN, TZ, NSEG, (SCHEME == 0 ? 4 : (SCHEME == 2 ? 3 : NY)), NUA1>(h, map, omap, a1, a2, p);
+    // stage 1 of the lean forms loads nothing but the stage input.  The DMA warp issues the store of item n - NUA before it
+    // goes on to the load of item n + 1, so its look-ahead is min(NY, NUA) items: 3 + 3 slots beat 4 + 2 (FD, HBM-bound)
+    case FIRST_LEAN: return launch_one<SCHEME, FIRST_LEAN, TZ, NSEG, (SCHEME == 1 ? NY : 3), (SCHEME == 0 ? 3 : NUA1)>(h, map, omap, a1, a2, p);   // KO r = 3 (halo 3): 3 + 2 is all that fits
     case LAST: return launch_one<SCHEME, LAST, TZ, NSEG, NY, NUA1>(h, map, omap, a1, a2, p);
     case MID_NOACC: return launch_one<SCHEME, MID_NOACC, TZ, NSEG, NY, NUA1>(h, map, omap, a1, a2, p);
     case LAST_P: return launch_one<SCHEME, LAST_P, TZ, NSEG, NY, NUA1>(h, map, omap, a1, a2, p);
@@ -704,8 +707,12 @@ extern "C" int cosenu_step(cosenu_t* h, int64_t n) {
                                   "(cosenu_slab_push_ghosts) first");
   CK(cudaSetDevice(h->device));
   if (h->use_graph && !h->slab && !h->stage_timing && n >= 2 * GRAPH_STEPS) {
-    if (!h->gexec) { int rc = build_graph(h); if (rc) return rc; }
-    for (; n >= GRAPH_STEPS; n -= GRAPH_STEPS) {
+    if (!h->gexec && build_graph(h) != COSENU_OK) {
+      // capture not possible here (e.g. a caller stream that is itself being captured): launch kernel by kernel from now on
+      (void)cudaGetLastError();
+      h->use_graph = 0;
+    }
+    for (; h->gexec && n >= GRAPH_STEPS; n -= GRAPH_STEPS) {
       CK(cudaGraphLaunch(h->gexec, h->stream));
       h->launches += 4 * GRAPH_STEPS; h->epoch += 4 * GRAPH_STEPS;
       h->step += GRAPH_STEPS;

@@ -339,6 +339,9 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
   //         (3) u0 / acc of item n into that slot (or just "slot is free" when the stage loads neither).
   if (warp == NW) {
     if (lane == 0) {
+      auto load_stream = [&](uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1) {   // operands without reuse
+        tma_load_3d(dst, map, bar, c0, c1, 0);
+      };
       auto store_item = [&](long long m) {   // outputs of item m
         const int su = (int)(m % NUA);
         const int iz0 = (int)(tile_of(blockIdx.x + (m / nchunks) * gridDim.x) * TZ), c0 = (int)(m % nchunks) * VC;
@@ -371,12 +374,11 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
         if constexpr (KT::NLOAD > 0) {
           mbar_expect_tx(b_full_ua + 8 * su, KT::NLOAD * SM::PTILE);
           const uint32_t dst = s_ua + su * NARR * SM::PTILE;
-          if constexpr (KT::LOAD_U0) tma_load_3d(dst, &tm_u0, b_full_ua + 8 * su, ch * VC, iz0, 0);
-          if constexpr (KT::LOAD_ACC)
-            tma_load_3d(dst + KT::ACC_LOAD_ARR * SM::PTILE, &tm_acc, b_full_ua + 8 * su, ch * VC, iz0, 0);
+          if constexpr (KT::LOAD_U0) load_stream(dst, &tm_u0, b_full_ua + 8 * su, ch * VC, iz0);
+          if constexpr (KT::LOAD_ACC) load_stream(dst + KT::ACC_LOAD_ARR * SM::PTILE, &tm_acc, b_full_ua + 8 * su, ch * VC, iz0);
           if constexpr (KT::LOAD_Y23) {
-            tma_load_3d(dst + SM::PTILE, &tm_acc, b_full_ua + 8 * su, ch * VC, iz0, 0);
-            tma_load_3d(dst + 2 * SM::PTILE, &tm_y3, b_full_ua + 8 * su, ch * VC, iz0, 0);
+            load_stream(dst + SM::PTILE, &tm_acc, b_full_ua + 8 * su, ch * VC, iz0);
+            load_stream(dst + 2 * SM::PTILE, &tm_y3, b_full_ua + 8 * su, ch * VC, iz0);
           }
         } else {
           mbar_arrive(b_full_ua + 8 * su);   // nothing to load: the slot is free for staging
