@@ -154,3 +154,12 @@ def test_fiducial_run_respects_the_light_cone(B, scheme):
     # waves propagate primarily toward +z: more converted flavour on the +z side of the centre
     pz = 1.0 - (st[0] / (st[0] + st[1]))                                         # rho_xx fraction per cell
     assert pz[zc > 0].sum() > pz[zc < 0].sum()
+
+
+@pytest.mark.parametrize("scheme", [FD, FV])
+def test_boxcar_advection_paper_setup(B, scheme):
+    """PAPER.md:180-185 at the paper's size and length (N_z = 2000 and 4000, C_CFL = 0.2, v = 0.5, t = 600): max error ~ 0.5,
+    unchanged with resolution; E2 drops; Gibbs oscillations for FD only."""
+    from test_oracle_pins import boxcar_run, check_boxcar
+    mk = lambda nz, nv, L, dt, s: B.Cosenu(nz, nv, L, dt, 0.0, 0.0, 0.0, s)
+    check_boxcar([boxcar_run(mk, scheme, nz, T=600.0) for nz in (2000, 4000)], scheme)

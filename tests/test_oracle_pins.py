@@ -651,3 +651,52 @@ def test_fiducial_seed_stays_inside_the_light_cone(scheme):
     assert ex[np.abs(zc) > t_end + 60.0].max() < 1e-12
     pz = 1.0 - st[0] / (st[0] + st[1])
     assert pz[zc > 0].sum() > pz[zc < 0].sum()            # forward-peaked angular distributions: waves go to +z
+
+
+# ----------------------------------------------------------------------------- box-car advection (Eq. 16, Fig. 3)
+def boxcar_run(make_sim, scheme, nz, T, L=1200.0, cfl=0.2):
+    """Advect the box of Eq. (16) with the beam v = +0.5 (N_v = 2 bin centres are -0.5, +0.5) on a
+    periodic domain of length L; returns (max |error|, E2, max u, min u, mass defect) at time T."""
+    nv = 2
+    dz = L / nz
+    dt = cfl * dz
+    z = (np.arange(nz) + (0.5 if scheme == FV else 0.0)) * dz - 0.5 * L
+    half = float(read_golden("paper_values.txt")["boxcar_half_width"])
+
+    def box(zz):
+        w = np.mod(zz + 0.5 * L, L) - 0.5 * L
+        return ((w >= -half) & (w <= half)).astype(float)
+
+    st = np.zeros((8, nz, nv))
+    st[0] = box(z)[:, None]
+    sim = make_sim(nz, nv, L, dt, scheme)
+    sim.set_state(st)
+    sim.step(int(round(T / dt)))
+    y = sim.get_state()[0][:, 1]
+    sim.close()
+    err = np.abs(y - box(z - 0.5 * T))
+    return err.max(), np.sqrt(np.mean(err ** 2)), y.max(), y.min(), abs(y.sum() - st[0][:, 1].sum()) * dz
+
+
+def check_boxcar(results, scheme):
+    """results: [(max err, E2, max, min, mass defect)] for increasing N_z."""
+    want = float(read_golden("paper_values.txt")["boxcar_max_error"])           # "~ 0.5" (PAPER.md:185)
+    for r in results:
+        assert abs(r[0] - want) < 0.2                                            # the jump is smeared over a few cells
+        assert r[4] < 1e-10                                                      # both schemes conserve the integral
+    # "remains unchanged" with resolution: it does not shrink (it moves within 0.35-0.6 with the position of the exact edge
+    # between two grid points)
+    assert abs(results[0][0] - results[-1][0]) < 0.2 and results[-1][0] > 0.3
+    assert results[-1][1] < 0.85 * results[0][1]                                # "E2 can be reduced with larger N_z"
+    if scheme == FD:
+        assert results[-1][2] > 1.05 and results[-1][3] < -0.05                 # Gibbs oscillations of the FD scheme
+    else:
+        assert results[-1][2] < 1.0 + 1e-3 and results[-1][3] > -1e-3           # WENO: essentially non-oscillatory (FD: 0.15)
+
+
+@pytest.mark.parametrize("scheme", [FD, FV])
+def test_boxcar_advection_error_is_half_and_resolution_independent(scheme):
+    """PAPER.md:180-185 (Fig. 3): max error ~ 0.5 for both schemes whatever the resolution, E2 drops with N_z, FD shows
+    Gibbs oscillations, FV does not.  (Domain length not printed: 1200, i.e. dz = 0.6 at the paper's N_z = 2000.)"""
+    mk = lambda nz, nv, L, dt, s: R.RefSim(nz, nv, L, dt, 0.0, 0.0, 0.0, s)
+    check_boxcar([boxcar_run(mk, scheme, nz, T=90.0) for nz in (500, 1000)], scheme)
