@@ -163,3 +163,22 @@ def test_boxcar_advection_paper_setup(B, scheme):
     from test_oracle_pins import boxcar_run, check_boxcar
     mk = lambda nz, nv, L, dt, s: B.Cosenu(nz, nv, L, dt, 0.0, 0.0, 0.0, s)
     check_boxcar([boxcar_run(mk, scheme, nz, T=600.0) for nz in (2000, 4000)], scheme)
+
+
+def test_fd_without_ko_dissipation_turns_unphysical(B):
+    """PAPER.md:269-271 (Fig. 7): in the fiducial run "the FD simulation without dissipation leads to numerical instabilities
+    starting at t ~ 800 ... and produces unphysically large values of P_3 > 1", which the Kreiss-Oliger term (eps_KO = 0.1)
+    and the FV scheme do not.  P_3 = (rho_ee - rho_xx) / (rho_ee + rho_xx) per cell.  (Domain length not printed: 1200.)"""
+    nz, nv, L = 2000, 100, 1200.0
+    dz = L / nz
+    dt = 0.2 * dz
+    worst = {}
+    for name, scheme, eps in (("fd_no_ko", FD, 0.0), ("fd_ko", FD, 0.1), ("fv", FV, None)):
+        g = B.Cosenu(nz, nv, L, dt, 0.0, 0.0, 1.0, scheme, eps_ko=eps)
+        g.init(1, pert_amp=1e-2, pert_kind=2)
+        g.step(int(round(800.0 / dt)))
+        st = g.get_state()
+        g.close()
+        worst[name] = max(np.abs((st[0] - st[1]) / (st[0] + st[1])).max(), np.abs((st[4] - st[5]) / (st[4] + st[5])).max())
+    assert worst["fd_no_ko"] > 1.0 + 1e-3, worst
+    assert worst["fd_ko"] < 1.0 + 1e-6 and worst["fv"] < 1.0 + 1e-6, worst
