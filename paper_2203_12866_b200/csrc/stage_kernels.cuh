@@ -20,6 +20,12 @@
 //    (xfull/xfree mbarriers); the tile's left boundary flux is split by component over 8 warps.
 //  * Moments of the output: butterfly reduce-scatter over the lanes (N values cost ~N adds, not 5N),
 //    accumulated over the chunks in registers of the owning lanes in fixed order => bit-reproducible.
+//  * Tile heights: TZ = 16 (S = 2 rows per warp) or, for the WENO7 kinds that stage one array, TZ = 24 (S = 3: the
+//    undivided differences are shared by three interfaces, weno7_face3).  SCHEME 2 = FD4 + KO of order r = 3 (halo 3).
+//  * Ghost rows / z-slabs: the warps that produce the first / last G rows also store their ghost copies -- into this
+//    buffer (periodic domain) or into the neighbouring slab's buffer over peer memory, followed by a release-add on
+//    the neighbour's arrival counter; the DMA warp acquires its own counters before it loads a tile that touches ghost
+//    rows.
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
