@@ -49,7 +49,7 @@ NCU_TRAFFIC_BYTES = {("cfg4", 2): 44279386880, ("cfg3", 2): 10752631296,   # pro
 # fp64 instructions (DFMA + DMUL + DADD, per thread = per (z,v) cell) one stage launch executes per cell, from
 # smsp__sass_thread_inst_executed_op_d{fma,mul,add}_pred_on.sum of the committed capture (profiles/r01b_fp64_*.csv): the
 # ALU side of the roofline.  Peak = 148 SMs x 4 sub-partitions x 16 fp64 lanes per clock x 1.965 GHz.
-FP64_PER_CELL = {"WENO7": {"FIRST_LEAN": 602.5, "MID_P": 663.4, "MID_NOACC": 602.5, "LAST_P": 610.5},
+FP64_PER_CELL = {"WENO7": {"FIRST_LEAN": 594.1, "MID_P": 654.9, "MID_NOACC": 594.1, "LAST_P": 602.1},
                  "FD4_KO3": {"FIRST_LEAN": 151.9, "MID_P": 175.9, "MID_NOACC": 151.9, "LAST_P": 159.9}}
 FP64_PEAK_LANE_OPS = 148 * 4 * 16 * 1.965e9
 

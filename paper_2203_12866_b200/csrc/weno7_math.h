@@ -46,18 +46,21 @@ using std::fma;
 
 namespace cosenu_math {
 
-// reciprocal: hardware seed (MUFU.RCP64H) + 2 Newton steps on the device (~1 ulp), plain division on the host
-COSENU_HD double fast_rcp2(double d) {
+// 1/(2d): hardware seed (MUFU.RCP64H) + 2 Newton steps on the device (~1 ulp), plain division on the host.  The factor 1/2
+// of "F = u_i + (1/2) num/den" costs no fp64 instruction: 2d is an exponent increment (integer add on the high word), and
+// every quantity of the iteration is then an exact power-of-two multiple of the plain reciprocal's.  d > 0, finite, normal.
+COSENU_HD double fast_half_rcp(double d) {
 #ifdef __CUDA_ARCH__
+  const double d2 = __hiloint2double(__double2hiint(d) + 0x00100000, __double2loint(d));
   double x;
-  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(d));
-  double e = fma(-d, x, 1.0);
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(d2));
+  double e = fma(-d2, x, 1.0);
   x = fma(x, e, x);
-  e = fma(-d, x, 1.0);
+  e = fma(-d2, x, 1.0);
   x = fma(x, e, x);
   return x;
 #else
-  return 1.0 / d;
+  return 0.5 / d;
 #endif
 }
 
@@ -105,7 +108,7 @@ COSENU_HD double weno7_core(double ui, double D0, double D1, double D2, double D
                c3 = fma(1.0 / 6.0, s3, A3);
   const double den = fma(Q01, Q2 + Q3, Q23 * (Q0 + Q1));
   const double num = fma(Q01, fma(Q3, c2, Q2 * c3), Q23 * fma(Q1, c0, Q0 * c1));
-  return fma(num, 0.5 * fast_rcp2(den), ui);
+  return fma(num, fast_half_rcp(den), ui);
 }
 
 // WENO7 value of u at the interface between w[3] and w[4], biased towards w[0] (the upwind side):
