@@ -43,7 +43,7 @@ STAGE_KERNEL = {0: ["FIRST", "MID", "MID", "LAST"], 1: ["FIRST_LEAN", "MID_REBUI
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant stage launch from the
 # committed ncu capture (profiles/r01_traffic_*.csv), per (workload, rk_form); None where not captured
 NCU_TRAFFIC_BYTES = {("cfg4", 2): 44279386880, ("cfg3", 2): 10752631296,   # profiles/r01_traffic_*.csv, RK stage 4 (LAST_COMB)
-                     ("cfg4", 3): 34646612224, ("cfg3", 3): 8673679872}    # profiles/r01b_traffic_*.csv, RK stage 2 (MID_P)
+                     ("cfg4", 3): 34648798208, ("cfg3", 3): 8662183168}    # profiles/r01b_traffic_*.csv, RK stage 2 (MID_P)
 
 
 # fp64 instructions (DFMA + DMUL + DADD, per thread = per (z,v) cell) one stage launch executes per cell, from
