@@ -168,3 +168,14 @@ def test_analysis_dP_map_matches_the_diagnostics_definition():
     assert abs(m - d["dP_max"]) <= 1e-13
     assert analysis.dP_map(st0, st0).max() <= 1e-12      # 1e-6 seed: |P| is uniform in z to O(1e-12) at t = 0
     r.close()
+
+
+def test_analysis_estimators_on_known_sequences():
+    """E2 (Eq. 15), the order estimator (Eq. C.3) and kappa (Eq. 24) on sequences whose answers are known."""
+    from paper_2203_12866_b200 import analysis
+    assert abs(analysis.e2_norm([1.0, 2.0, 3.0], [1.0, 2.0, 5.0]) - np.sqrt(4.0 / 3.0)) < 1e-15
+    for p in (3.0, 4.0, 7.0):
+        assert abs(analysis.order_of_convergence(5.0, 5.0 / 2 ** p) - p) < 1e-12          # errors ~ h^p, h halved
+        q = [1.0 + 0.3 * h ** p for h in (0.4, 0.2, 0.1)]                                   # q(h) = q* + C h^p
+        assert abs(analysis.kappa(*q) - 2 ** p) < 1e-6 * 2 ** p                             # kappa -> 2^p
+    assert analysis.kappa(1.0, 2.0, 2.0) == float("inf")
