@@ -534,7 +534,7 @@ int build_graph(cosenu* h) {
 namespace {
 cosenu* create_common(int64_t nz_global, int64_t z_begin, int64_t nz, int32_t nv, double L, double dt, double omega,
                       double theta, double mu, int scheme, bool slab) {
-  if (nz < 16 || nz > 2000000000ll || nz_global < nz || nz_global > 2000000000ll || z_begin < 0 || z_begin >= nz_global ||
+  if (nz < 16 || nz > 2000000000ll || nz_global < nz || nz_global > 2000000000ll || z_begin < 0 || z_begin + nz > nz_global ||
       nv < 2 || nv > (1 << 20) || !(L > 0) || !(dt > 0) || (scheme != 0 && scheme != 1) || !std::isfinite(L) ||
       !std::isfinite(dt) || !std::isfinite(omega) || !std::isfinite(theta) || !std::isfinite(mu)) {
     g_create_err = "cosenu_create: invalid argument";

@@ -139,6 +139,8 @@ def test_slab_call_order_errors(B, S):
         B.Cosenu(8, 8, 64.0, 0.1, 0, 0, 1.0, FD, slab=(128, 0))        # thinner than 16 rows
     with pytest.raises(B.CosenuError):
         B.Cosenu(64, 8, 64.0, 0.1, 0, 0, 1.0, FD, slab=(32, 0))        # larger than the grid
+    with pytest.raises(B.CosenuError):
+        B.Cosenu(64, 8, 64.0, 0.1, 0, 0, 1.0, FD, slab=(128, 100))     # sticks out of the grid
 
 
 # ---------------------------------------------------------------------------------------------------------
