@@ -88,3 +88,38 @@ def test_cfg2_long_run_against_stored_oracle_series():
           % (done, worst, first_bad))
     print("  step, |dPsurv|, Psurv_gpu: " + "; ".join("%d %.2e %.6f" % r for r in report[::max(1, len(report) // 12)]))
     assert worst <= 1e-6, (worst, first_bad)
+
+
+@pytest.mark.parametrize("name", ["cfg3", "cfg4"])
+def test_bandwidth_scale_configs_over_their_full_length(name):
+    """BASELINE configs 3 (200 steps) and 4 (100 steps) at full size: what must hold at any size and length --
+    the trace of every cell stays put (the commutator is traceless, the initial state is z-homogeneous), the lepton-number
+    vector M0 is conserved (its projection on B-hat when the vacuum term is on, PAPER.md:247-249 / DESIGN R2), the
+    survival probability stays in [0, 1], no NaN; and the state is reproduced bit for bit by a second run."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2203_12866_b200 import binding as B
+    c = inputs.CONFIGS[name]
+    free, _ = torch.cuda.mem_get_info()
+    if free < 5 * 64 * c["nz"] * c["nv"]:
+        pytest.skip("not enough device memory")
+    out = []
+    for _ in range(2):
+        g = B.Cosenu(c["nz"], c["nv"], c["L"], c["dt"], c["omega"], c["theta"], c["mu"], c["scheme"])
+        g.init(c["seed"])
+        g.step(c["steps"])
+        d = g.diagnostics()
+        m = g.get_moments()
+        g.close()
+        out.append((d, m))
+    d, m = out[0]
+    assert d["step"] == c["steps"] and np.isfinite(m).all()
+    assert d["trace_dev_max"] <= 1e-12
+    assert 0.0 < d["psurv_nu"] <= 1.0 + 1e-12 and 0.0 < d["psurv_nubar"] <= 1.0 + 1e-12
+    s2, c2 = np.sin(2 * c["theta"]), np.cos(2 * c["theta"])
+    along_B = s2 * d["dM0"][0] - c2 * d["dM0"][2]
+    assert abs(along_B) <= 1e-9 * c["nz"]
+    if c["omega"] == 0.0:
+        assert max(abs(x) for x in d["dM0"]) <= 1e-9 * c["nz"]
+    assert np.array_equal(m, out[1][1]) and d == out[1][0]          # deterministic summation order: bitwise repeatable
