@@ -180,7 +180,8 @@ def test_slabs_in_separate_processes_over_cuda_ipc(B, scheme, world):
     ref, _, refd = _single(B, args, st, nsteps)
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
-    port = 29620 + 3 * scheme + world
+    from conftest import free_port
+    port = free_port()
     ps = [ctx.Process(target=_ipc_worker, args=(r, world, port, nz, nv, scheme, nsteps, q)) for r in range(world)]
     for p in ps:
         p.start()

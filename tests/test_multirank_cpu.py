@@ -25,9 +25,11 @@ def _worker(rank, world, port, q):
 
 
 def test_max_over_ranks_and_aggregate_gloo():
+    from conftest import free_port
+    port = free_port()
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
-    ps = [ctx.Process(target=_worker, args=(r, 2, 29613, q)) for r in range(2)]
+    ps = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
     for p in ps:
         p.start()
     out = sorted(q.get(timeout=120) for _ in ps)
@@ -97,10 +99,12 @@ def _slab_worker(rank, world, port, q):
 
 def test_slab_ring_plumbing_gloo():
     import numpy as np
+    from conftest import free_port
+    port = free_port()
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
     world = 2
-    ps = [ctx.Process(target=_slab_worker, args=(r, world, 29617, q)) for r in range(world)]
+    ps = [ctx.Process(target=_slab_worker, args=(r, world, port, q)) for r in range(world)]
     for p in ps:
         p.start()
     out = sorted(q.get(timeout=120) for _ in ps)
