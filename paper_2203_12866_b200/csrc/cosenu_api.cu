@@ -29,7 +29,8 @@ typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_
 // tile shapes: TZ rows per tile, NSEG compute warps (S = TZ/NSEG rows each),
 // NY / NUA ring depths of the stage-input and of the u0/acc shared-memory slots.  `variant` picks a row.
 constexpr int TZ_ALL = 16;
-constexpr int TZ_WENO1 = 24;   // WENO7, kinds that stage one array: 3 rows per warp (shared differences, fewer boundary fluxes)
+constexpr int TZ_WENO1 = 24;   // WENO7, kinds that stage one array: 12 compute warps x 2 rows
+constexpr int TZ_WENO2 = 22;   // ... 11 compute warps x 2 rows (the kind that needs more than 128 registers)
 constexpr int DIAG_BLOCKS = 592, DIAG_THREADS = 256, REF_BLOCKS = 148;
 
 std::string g_create_err;
@@ -58,10 +59,10 @@ struct cosenu {
   double *d_pref = nullptr, *d_p0ref = nullptr, *d_refpart = nullptr, *d_diagpart = nullptr;
   int64_t comp_stride = 0; size_t state_elems = 0;
   int mcur = 0;  // M[mcur] holds the moments of U
-  // tensor maps per tile height (index 0: TZ = 16, 1: TZ = 24 [WENO7 kinds that stage one array]) and per state buffer
+  // tensor maps per tile height (index 0: TZ = 16, 1: TZ = 24, 2: TZ = 22 [WENO7 kinds that stage one array]) and per state buffer
   // (0 U, 1 Y1, 2 Y2, 3 ACC)
-  CUtensorMap tm[2][4];   // stage-input boxes [8][TZ+2H][32] over the ghosted rows
-  CUtensorMap tp[2][4];   // rows 0..nz-1 only, boxes [8][TZ][32]: u0 / acc loads, output stores
+  CUtensorMap tm[3][4];   // stage-input boxes [8][TZ+2H][32] over the ghosted rows
+  CUtensorMap tp[3][4];   // rows 0..nz-1 only, boxes [8][TZ][32]: u0 / acc loads, output stores
   bool maps_ready = false;
 
   bool have_state = false;
@@ -188,9 +189,9 @@ int make_maps(cosenu* h) {
   PFN_encodeTiled enc = reinterpret_cast<PFN_encodeTiled>(fn);
   const int halo = h->scheme == COSENU_FD4_KO3 ? h->ko_r : 4;
   double* bufs[4] = {h->U, h->Y1, h->Y2, h->ACC};
-  const int tzs[2] = {TZ_ALL, TZ_WENO1};
-  for (int t = 0; t < 2; ++t) {
-    if (t == 1 && h->scheme != COSENU_FV_WENO7) continue;
+  const int tzs[3] = {TZ_ALL, TZ_WENO1, TZ_WENO2};
+  for (int t = 0; t < 3; ++t) {
+    if (t >= 1 && h->scheme != COSENU_FV_WENO7) continue;
     for (int b = 0; b < 4; ++b) {
       int rc;
       if ((rc = make_map(h, enc, &h->tm[t][b], bufs[b], tzs[t] + 2 * halo, true))) return rc;
@@ -202,7 +203,7 @@ int make_maps(cosenu* h) {
 
 template <int SCHEME, int KIND, int TZ, int NSEG, int NY, int NUA>
 int launch_one(cosenu* h, int in_buf, int out_buf, int a1_buf, int a2_buf, const StageParams& p0) {
-  constexpr int T = TZ == TZ_ALL ? 0 : 1;
+  constexpr int T = TZ == TZ_ALL ? 0 : (TZ == TZ_WENO1 ? 1 : 2);
   const CUtensorMap &map = h->tm[T][in_buf], &omap = h->tp[T][out_buf], &a1 = h->tp[T][a1_buf], &a2 = h->tp[T][a2_buf];
   auto kern = stage_kernel<SCHEME, KIND, TZ, NSEG, NY, NUA>;
   constexpr size_t smem = StageSmem<SCHEME, KIND, TZ, NSEG, NY, NUA>::bytes;
@@ -259,15 +260,24 @@ int launch_stage(cosenu* h, int kind, int map, int omap, int a1, int a2, const S
     return launch_kind<0, TZ_ALL, 8, 2, 2>(h, kind, map, omap, a1, a2, p);
   }
   if (h->variant == 1) return launch_kind<1, TZ_ALL, 16, 2, 1>(h, kind, map, omap, a1, a2, p);
-  // the kinds that stage one array leave room for tiles of 24 rows = 3 rows per warp: the undivided differences are
-  // shared by three interfaces and the tile-boundary flux is recomputed once per 24 rows instead of 16
-  // ... unless the coarser tiles quantise worse over the persistent grid (rows walked by the busiest CTA; the taller
-  // tile is worth about 2 %): e.g. nz = 32768 is 13.8 waves of 16-row tiles but 9.2 waves of 24-row tiles
+  // the kinds that stage one array leave room for taller tiles and more compute warps, unless the coarser tiles quantise
+  // worse over the persistent grid (rows walked by the busiest CTA): e.g. nz = 32768 is 13.8 waves of 16-row tiles but
+  // 9.2 waves of 24-row tiles
   const long long w16 = ((h->nz + TZ_ALL - 1) / TZ_ALL + h->num_sms - 1) / h->num_sms * TZ_ALL;
   const long long w24 = ((h->nz + TZ_WENO1 - 1) / TZ_WENO1 + h->num_sms - 1) / h->num_sms * TZ_WENO1;
-  const bool tz24 = h->variant == 2 || (h->variant == 0 && 0.98 * (double)w24 <= (double)w16);   // variant 3: never
-  if (tz24 && (kind == FIRST_LEAN || kind == MID_NOACC || kind == LAST_P || kind == LAST))
-    return launch_kind<1, TZ_WENO1, 8, 2, 1>(h, kind, map, omap, a1, a2, p);
+  const bool tz24 = h->variant == 2 || (h->variant == 0 && 0.93 * (double)w24 <= (double)w16);   // variant 3: never
+  if (tz24) {
+    // Three compute warps per scheduler instead of two hide the fp64 latencies much better (FP64 pipe 81 % busy instead of
+    // 71 %): 12 warps x 2 rows on 24-row tiles.  13 warps cap the kernel at 128 registers, which MID_NOACC does not fit
+    // without spilling in its hot loop: that kind runs 11 warps x 2 rows on 22-row tiles (12 warps in all, 166 registers).
+    switch (kind) {
+      case FIRST_LEAN: return launch_one<1, FIRST_LEAN, TZ_WENO1, 12, 2, 1>(h, map, omap, a1, a2, p);
+      case LAST_P: return launch_one<1, LAST_P, TZ_WENO1, 12, 2, 1>(h, map, omap, a1, a2, p);
+      case MID_NOACC: return launch_one<1, MID_NOACC, TZ_WENO2, 11, 2, 1>(h, map, omap, a1, a2, p);
+      case LAST: return launch_one<1, LAST, TZ_WENO2, 11, 2, 1>(h, map, omap, a1, a2, p);
+      default: break;
+    }
+  }
   return launch_kind<1, TZ_ALL, 8, 2, 1>(h, kind, map, omap, a1, a2, p);
 }
 
