@@ -43,13 +43,13 @@ STAGE_KERNEL = {0: ["FIRST", "MID", "MID", "LAST"], 1: ["FIRST_LEAN", "MID_REBUI
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant stage launch from the
 # committed ncu capture (profiles/r01_traffic_*.csv), per (workload, rk_form); None where not captured
 NCU_TRAFFIC_BYTES = {("cfg4", 2): 44279386880, ("cfg3", 2): 10752631296,   # profiles/r01_traffic_*.csv, RK stage 4 (LAST_COMB)
-                     ("cfg4", 3): 34648798208, ("cfg3", 3): 8662183168}    # profiles/r01b_traffic_*.csv, RK stage 2 (MID_P)
+                     ("cfg4", 3): 34396154624, ("cfg3", 3): 8674394880}    # profiles/r01b_traffic_*.csv, RK stage 2 (MID_P)
 
 
 # fp64 instructions (DFMA + DMUL + DADD, per thread = per (z,v) cell) one stage launch executes per cell, from
 # smsp__sass_thread_inst_executed_op_d{fma,mul,add}_pred_on.sum of the committed capture (profiles/r01b_fp64_*.csv): the
 # ALU side of the roofline.  Peak = 148 SMs x 4 sub-partitions x 16 fp64 lanes per clock x 1.965 GHz.
-FP64_PER_CELL = {"WENO7": {"FIRST_LEAN": 594.1, "MID_P": 654.9, "MID_NOACC": 594.1, "LAST_P": 602.1},
+FP64_PER_CELL = {"WENO7": {"FIRST_LEAN": 618.3, "MID_P": 647.2, "MID_NOACC": 620.5, "LAST_P": 626.3},
                  "FD4_KO3": {"FIRST_LEAN": 151.9, "MID_P": 175.9, "MID_NOACC": 151.9, "LAST_P": 159.9}}
 FP64_PEAK_LANE_OPS = 148 * 4 * 16 * 1.965e9
 

@@ -30,6 +30,7 @@ typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_
 // NY / NUA ring depths of the stage-input and of the u0/acc shared-memory slots.  `variant` picks a row.
 constexpr int TZ_ALL = 16;
 constexpr int TZ_WENO1 = 24;   // WENO7, kinds that stage one array: 12 compute warps x 2 rows
+constexpr int TZ_WENO3 = 20;   // ... 10 compute warps x 2 rows: stage 2 of RK form 3, which stages two arrays
 constexpr int TZ_WENO2 = 22;   // ... 11 compute warps x 2 rows (the kind that needs more than 128 registers)
 constexpr int DIAG_BLOCKS = 592, DIAG_THREADS = 256, REF_BLOCKS = 148;
 
@@ -59,10 +60,10 @@ struct cosenu {
   double *d_pref = nullptr, *d_p0ref = nullptr, *d_refpart = nullptr, *d_diagpart = nullptr;
   int64_t comp_stride = 0; size_t state_elems = 0;
   int mcur = 0;  // M[mcur] holds the moments of U
-  // tensor maps per tile height (index 0: TZ = 16, 1: TZ = 24, 2: TZ = 22 [WENO7 kinds that stage one array]) and per state buffer
+  // tensor maps per tile height (index 0: TZ = 16; WENO7 only: 1: TZ = 24, 2: TZ = 22, 3: TZ = 20) and per state buffer
   // (0 U, 1 Y1, 2 Y2, 3 ACC)
-  CUtensorMap tm[3][4];   // stage-input boxes [8][TZ+2H][32] over the ghosted rows
-  CUtensorMap tp[3][4];   // rows 0..nz-1 only, boxes [8][TZ][32]: u0 / acc loads, output stores
+  CUtensorMap tm[4][4];   // stage-input boxes [8][TZ+2H][32] over the ghosted rows
+  CUtensorMap tp[4][4];   // rows 0..nz-1 only, boxes [8][TZ][32]: u0 / acc loads, output stores
   bool maps_ready = false;
 
   bool have_state = false;
@@ -189,8 +190,8 @@ int make_maps(cosenu* h) {
   PFN_encodeTiled enc = reinterpret_cast<PFN_encodeTiled>(fn);
   const int halo = h->scheme == COSENU_FD4_KO3 ? h->ko_r : 4;
   double* bufs[4] = {h->U, h->Y1, h->Y2, h->ACC};
-  const int tzs[3] = {TZ_ALL, TZ_WENO1, TZ_WENO2};
-  for (int t = 0; t < 3; ++t) {
+  const int tzs[4] = {TZ_ALL, TZ_WENO1, TZ_WENO2, TZ_WENO3};
+  for (int t = 0; t < 4; ++t) {
     if (t >= 1 && h->scheme != COSENU_FV_WENO7) continue;
     for (int b = 0; b < 4; ++b) {
       int rc;
@@ -203,7 +204,7 @@ int make_maps(cosenu* h) {
 
 template <int SCHEME, int KIND, int TZ, int NSEG, int NY, int NUA>
 int launch_one(cosenu* h, int in_buf, int out_buf, int a1_buf, int a2_buf, const StageParams& p0) {
-  constexpr int T = TZ == TZ_ALL ? 0 : (TZ == TZ_WENO1 ? 1 : 2);
+  constexpr int T = TZ == TZ_ALL ? 0 : (TZ == TZ_WENO1 ? 1 : (TZ == TZ_WENO2 ? 2 : 3));
   const CUtensorMap &map = h->tm[T][in_buf], &omap = h->tp[T][out_buf], &a1 = h->tp[T][a1_buf], &a2 = h->tp[T][a2_buf];
   auto kern = stage_kernel<SCHEME, KIND, TZ, NSEG, NY, NUA>;
   constexpr size_t smem = StageSmem<SCHEME, KIND, TZ, NSEG, NY, NUA>::bytes;
@@ -275,6 +276,7 @@ int launch_stage(cosenu* h, int kind, int map, int omap, int a1, int a2, const S
       case LAST_P: return launch_one<1, LAST_P, TZ_WENO1, 12, 2, 1>(h, map, omap, a1, a2, p);
       case MID_NOACC: return launch_one<1, MID_NOACC, TZ_WENO2, 11, 2, 1>(h, map, omap, a1, a2, p);
       case LAST: return launch_one<1, LAST, TZ_WENO2, 11, 2, 1>(h, map, omap, a1, a2, p);
+      case MID_P: return launch_one<1, MID_P, TZ_WENO3, 10, 2, 1>(h, map, omap, a1, a2, p);   // two staged arrays: 20 rows is what fits
       default: break;
     }
   }

@@ -20,8 +20,9 @@
 //    (xfull/xfree mbarriers); the tile's left boundary flux is split by component over 8 warps.
 //  * Moments of the output: butterfly reduce-scatter over the lanes (N values cost ~N adds, not 5N),
 //    accumulated over the chunks in registers of the owning lanes in fixed order => bit-reproducible.
-//  * Tile heights: TZ = 16 (S = 2 rows per warp) or, for the WENO7 kinds that stage one array, TZ = 24 (S = 3: the
-//    undivided differences are shared by three interfaces, weno7_face3).  SCHEME 2 = FD4 + KO of order r = 3 (halo 3).
+//  * Tile heights and warps: TZ = 16 with 8 compute warps x 2 rows everywhere, except the WENO7 kernels of the default RK
+//    form, which run three compute warps per scheduler as far as shared memory and registers allow: 12 warps x 2 rows
+//    (TZ = 24), 11 x 2 (TZ = 22) or, with two staged arrays, 10 x 2 (TZ = 20).  SCHEME 2 = FD4 + KO of order r = 3 (halo 3).
 //  * Ghost rows / z-slabs: the warps that produce the first / last G rows also store their ghost copies -- into this
 //    buffer (periodic domain) or into the neighbouring slab's buffer over peer memory, followed by a release-add on
 //    the neighbour's arrival counter; the DMA warp acquires its own counters before it loads a tile that touches ghost
@@ -240,7 +241,7 @@ __device__ __forceinline__ void butterfly_reduce(double (&x)[N], int lane, int& 
 // FR[s][c] = WENO7 value of u_c at the right interface of row (rel_row + s).
 template <int DIR, int S, int ROWS, int H>
 __device__ __forceinline__ void weno_rows(uint32_t Tw, const cosenu_math::Weno7Beam& bm, double (&FR)[S][8]) {
-  static_assert(S == 1 || S == 2 || S == 3, "rows per warp");
+  static_assert(S == 1 || S == 2, "rows per warp");
 #pragma unroll
   for (int c = 0; c < 8; ++c) {
     if constexpr (S == 1) {
@@ -248,22 +249,13 @@ __device__ __forceinline__ void weno_rows(uint32_t Tw, const cosenu_math::Weno7B
 #pragma unroll
       for (int k = 0; k < 7; ++k) w[k] = lds(Tw + ((c * ROWS + H + (DIR > 0 ? 0 : 1) + DIR * (k - 3)) * VC) * 8);
       FR[0][c] = cosenu_math::weno7_face(w, bm);
-    } else if constexpr (S == 2) {
+    } else {
       double w[8], Fa, Fb;
 #pragma unroll
       for (int k = 0; k < 8; ++k) w[k] = lds(Tw + ((c * ROWS + H + (DIR > 0 ? k - 3 : 5 - k)) * VC) * 8);
       cosenu_math::weno7_face2(w, bm, Fa, Fb);
       FR[DIR > 0 ? 0 : 1][c] = Fa;
       FR[DIR > 0 ? 1 : 0][c] = Fb;
-    } else {
-      // three rows per warp: 9 cells, the undivided differences are shared by the three interfaces
-      double w[9], Fa, Fb, Fc;
-#pragma unroll
-      for (int k = 0; k < 9; ++k) w[k] = lds(Tw + ((c * ROWS + H + (DIR > 0 ? k - 3 : 6 - k)) * VC) * 8);
-      cosenu_math::weno7_face3(w, bm, Fa, Fb, Fc);
-      FR[DIR > 0 ? 0 : 2][c] = Fa;
-      FR[1][c] = Fb;
-      FR[DIR > 0 ? 2 : 0][c] = Fc;
     }
   }
 }

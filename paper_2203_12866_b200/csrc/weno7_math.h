@@ -133,19 +133,6 @@ COSENU_HD void weno7_face2(const double w[8], const Weno7Beam& bm, double& Fa, d
   Fb = weno7_core(w[4], D1, D2, D3, D4, E1, E2, E3, E4, E5, T1, T4, TT1, TT2, TT3, TT4, bm);
 }
 
-// three adjacent interfaces from 9 cells w[0..8] with shared differences:
-//   Fa = w[3]|w[4],  Fb = w[4]|w[5],  Fc = w[5]|w[6], all biased towards w[0].
-COSENU_HD void weno7_face3(const double w[9], const Weno7Beam& bm, double& Fa, double& Fb, double& Fc) {
-  const double D0 = w[1] - w[0], D1 = w[2] - w[1], D2 = w[3] - w[2], D3 = w[4] - w[3], D4 = w[5] - w[4],
-               D5 = w[6] - w[5], D6 = w[7] - w[6], D7 = w[8] - w[7];
-  const double E0 = D1 - D0, E1 = D2 - D1, E2 = D3 - D2, E3 = D4 - D3, E4 = D5 - D4, E5 = D6 - D5, E6 = D7 - D6;
-  const double T0 = E1 - E0, T1 = E2 - E1, T2 = E3 - E2, T3 = E4 - E3, T4 = E5 - E4, T5 = E6 - E5;
-  const double TT0 = T0 * T0, TT1 = T1 * T1, TT2 = T2 * T2, TT3 = T3 * T3, TT4 = T4 * T4, TT5 = T5 * T5;
-  Fa = weno7_core(w[3], D0, D1, D2, D3, E0, E1, E2, E3, E4, T0, T3, TT0, TT1, TT2, TT3, bm);
-  Fb = weno7_core(w[4], D1, D2, D3, D4, E1, E2, E3, E4, E5, T1, T4, TT1, TT2, TT3, TT4, bm);
-  Fc = weno7_core(w[5], D2, D3, D4, D5, E2, E3, E4, E5, E6, T2, T5, TT2, TT3, TT4, TT5, bm);
-}
-
 // FD4 + KO3 in difference form (Eq. (5)): returns
 //   cadv * (u_{i-2} - 8u_{i-1} + 8u_{i+1} - u_{i+2}) + cko * (u_{i-2} - 4u_{i-1} + 6u_i - 4u_{i+1} + u_{i+2})
 // with cadv = -v/(12 dz), cko = -eps_ko/(16 dz) (dissipative sign, reading A4).
