@@ -17,6 +17,7 @@
 
 #include "aux_kernels.cuh"
 #include "stage_kernels.cuh"
+#include "weno_march.cuh"
 
 using namespace cosenu_dev;
 
@@ -226,6 +227,28 @@ int launch_one(cosenu* h, int in_buf, int out_buf, int a1_buf, int a2_buf, const
   return COSENU_OK;
 }
 
+// WENO7, partial-sum RK carrier: the role-specialised marching kernel (weno_march.cuh) on 16-row tiles
+template <int KIND>
+int launch_march(cosenu* h, int in_buf, int out_buf, int acc_buf, const StageParams& p0) {
+  auto kern = weno_march_kernel<KIND>;
+  constexpr size_t smem = MarchSmem::bytes;
+  static_assert(smem <= 232448, "over the 227 KB shared-memory limit of a CTA");
+  const void* key = reinterpret_cast<const void*>(kern);
+  if (h->configured.find(key) == h->configured.end()) {
+    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    h->configured.insert(key);
+  }
+  if (h->dry_run) return COSENU_OK;
+  const long long ntiles = (h->nz + MTZ - 1) / MTZ;
+  const unsigned grid = (unsigned)(ntiles < h->num_sms ? ntiles : h->num_sms);   // persistent: one CTA per SM
+  StageParams p = p0;
+  if (h->slab) p.tile_shift = ntiles >= 3 ? ntiles - 2 : 0;
+  kern<<<grid, MARCH_THREADS, smem, h->stream>>>(h->tm[0][in_buf], h->tp[0][0], h->tp[0][acc_buf], h->tp[0][out_buf], p);
+  CK(cudaGetLastError());
+  h->launches++;
+  return COSENU_OK;
+}
+
 template <int SCHEME, int TZ, int NSEG, int NY, int NUA, int NUA1 = NUA>   // NUA1: ring depth of the kinds that stage ONE array
 int launch_kind(cosenu* h, int kind, int map, int omap, int a1, int a2, const StageParams& p) {
   // kinds that stage ONE array (they also fit tiles of TZ_WENO1 rows)
@@ -261,6 +284,15 @@ int launch_stage(cosenu* h, int kind, int map, int omap, int a1, int a2, const S
     return launch_kind<0, TZ_ALL, 8, 2, 2>(h, kind, map, omap, a1, a2, p);
   }
   if (h->variant == 1) return launch_kind<1, TZ_ALL, 16, 2, 1>(h, kind, map, omap, a1, a2, p);
+  if (h->variant == 4) {
+    switch (kind) {
+      case FIRST_LEAN: return launch_march<FIRST_LEAN>(h, map, omap, a1, p);
+      case MID_P: return launch_march<MID_P>(h, map, omap, a1, p);
+      case MID_NOACC: return launch_march<MID_NOACC>(h, map, omap, a1, p);
+      case LAST_P: return launch_march<LAST_P>(h, map, omap, a1, p);
+      default: break;   // the other RK carriers run the row-block kernels below
+    }
+  }
   // the kinds that stage one array leave room for taller tiles and more compute warps, unless the coarser tiles quantise
   // worse over the persistent grid (rows walked by the busiest CTA): e.g. nz = 32768 is 13.8 waves of 16-row tiles but
   // 9.2 waves of 24-row tiles
@@ -613,7 +645,7 @@ extern "C" int cosenu_set_option(cosenu_t* h, int key, double value) {
     case COSENU_OPT_WENO_EPS: if (!(value > 0) || !(value <= 1e30)) break; h->weno_eps = value; return COSENU_OK;
     case COSENU_OPT_ADVECT: h->advect = value != 0; return COSENU_OK;
     case COSENU_OPT_RK_FORM: if (value != 0 && value != 1 && value != 2 && value != 3) break; h->rk_form = (int)value; return COSENU_OK;
-    case COSENU_OPT_VARIANT: if (value != 0 && value != 1 && value != 2 && value != 3) break; h->variant = (int)value; return COSENU_OK;
+    case COSENU_OPT_VARIANT: if (value != 0 && value != 1 && value != 2 && value != 3 && value != 4) break; h->variant = (int)value; return COSENU_OK;
     case COSENU_OPT_KO_ORDER:
       if (value != 2 && value != 3) break;
       if (h->ko_r != (int)value) {

@@ -202,26 +202,28 @@ struct StageSmem {
 // bit o keep the upper half and send the lower half (and vice versa), so N values cost about N adds and
 // N shuffles per lane instead of 5N.  On return x[0] of lane L holds the total of the original value
 // `idx` (if `valid`), idx = sum over stages of (lane bit ? half : 0).  Fixed tree => reproducible.
+// one stage (lane offset O, N live values -> (N + 1) / 2) and the stages below it; every index is a compile-time constant,
+// so the values stay in registers whatever N is
+template <int N, int O>
+__device__ __forceinline__ void butterfly_stage(double* x, int lane) {
+  constexpr int half = (N + 1) / 2;
+  const bool up = (lane & O) != 0;
+#pragma unroll
+  for (int i = 0; i < half; ++i) {
+    const double a = x[i];
+    const double b = (i + half < N) ? x[i + half] : 0.0;
+    const double send = up ? a : b;
+    const double keep = up ? b : a;
+    x[i] = keep + __shfl_xor_sync(0xffffffffu, send, O);
+  }
+  if constexpr (O > 1) butterfly_stage<half, O / 2>(x, lane);
+}
 template <int N>
 __device__ __forceinline__ void butterfly_reduce(double (&x)[N], int lane, int& idx, bool& valid) {
-  int n = N;
-#pragma unroll
-  for (int o = 16; o >= 1; o >>= 1) {
-    const int half = (n + 1) / 2;
-    const bool up = (lane & o) != 0;
-#pragma unroll
-    for (int i = 0; i < half; ++i) {
-      const double a = x[i];
-      const double b = (i + half < n) ? x[i + half] : 0.0;
-      const double send = up ? a : b;
-      const double keep = up ? b : a;
-      x[i] = keep + __shfl_xor_sync(0xffffffffu, send, o);
-    }
-    n = half;
-  }
+  butterfly_stage<N, 16>(x, lane);
   // which original index ended up in x[0] of this lane (replay the stages backwards)
   int ns[5], hs[5];
-  n = N;
+  int n = N;
 #pragma unroll
   for (int k = 0; k < 5; ++k) { ns[k] = n; hs[k] = (n + 1) / 2; n = hs[k]; }
   int pos = 0;
