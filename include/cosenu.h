@@ -62,10 +62,12 @@ enum {
                               default 3 */
   COSENU_OPT_STAGE_TIMING = 4, /* 1: bracket every stage launch with CUDA events on the handle's stream
                               (read with cosenu_stage_times); default 0 */
-  COSENU_OPT_VARIANT = 5,  /* kernel shape: 0 (default) = 8 compute warps x 2 rows on 16-row tiles; the WENO7 kernels of the default
-                              RK form use taller tiles with 10-12 compute warps x 2 rows when that does not quantise worse over
-                              the SMs; 1 = 16 compute warps x 1 row; 2 = as 0 with the tall tiles forced; 3 = as 0 without them.
-                              Same arithmetic per cell in all shapes */
+  COSENU_OPT_VARIANT = 5,  /* kernel shape (same arithmetic per cell in all shapes, bit-identical results):
+                              0 (default): FD: 8 compute warps x 2 rows on 16-row tiles.  WENO7 with the default RK form: the marching
+                                 kernel (csrc/weno_march.cuh: one warp per component marches along z through a 16-row tile, separate
+                                 warps combine); WENO7 with the other RK forms: the row-block kernel as in 3;
+                              1: 16 compute warps x 1 row;  2: row-block kernels, WENO7 on 20-24-row tiles with 10-12 compute warps;
+                              3: row-block kernels on 16-row tiles;  4: as 0 */
   COSENU_OPT_GRAPH = 8,    /* 1 (default): cosenu_step(n >= 16) replays a CUDA graph of 8 RK4 steps (32 kernel nodes) captured from the
                               handle's own launches, which removes the per-launch host cost on the small, launch-bound grids;
                               0: always launch kernel by kernel.  Not used on slab handles (their launch parameters change every

@@ -284,7 +284,7 @@ int launch_stage(cosenu* h, int kind, int map, int omap, int a1, int a2, const S
     return launch_kind<0, TZ_ALL, 8, 2, 2>(h, kind, map, omap, a1, a2, p);
   }
   if (h->variant == 1) return launch_kind<1, TZ_ALL, 16, 2, 1>(h, kind, map, omap, a1, a2, p);
-  if (h->variant == 4) {
+  if (h->variant == 0 || h->variant == 4) {   // default: the marching kernel (weno_march.cuh) for the kinds of the partial-sum RK carrier
     switch (kind) {
       case FIRST_LEAN: return launch_march<FIRST_LEAN>(h, map, omap, a1, p);
       case MID_P: return launch_march<MID_P>(h, map, omap, a1, p);

@@ -46,7 +46,8 @@ using std::fma;
 
 namespace cosenu_math {
 
-// 1/(2d): hardware seed (MUFU.RCP64H) + 2 Newton steps on the device (~1 ulp), plain division on the host.  The factor 1/2
+// 1/(2d): hardware seed (MUFU.RCP64H) + one third-order step (3 FMA instead of the 4 of two Newton steps; relative error
+// <= |e|^3 ~ 2^-57 + rounding) on the device, plain division on the host.  The factor 1/2
 // of "F = u_i + (1/2) num/den" costs no fp64 instruction: 2d is an exponent increment (integer add on the high word), and
 // every quantity of the iteration is then an exact power-of-two multiple of the plain reciprocal's.  d > 0, finite, normal.
 COSENU_HD double fast_half_rcp(double d) {
@@ -54,11 +55,9 @@ COSENU_HD double fast_half_rcp(double d) {
   const double d2 = __hiloint2double(__double2hiint(d) + 0x00100000, __double2loint(d));
   double x;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(d2));
-  double e = fma(-d2, x, 1.0);
-  x = fma(x, e, x);
-  e = fma(-d2, x, 1.0);
-  x = fma(x, e, x);
-  return x;
+  const double e = fma(-d2, x, 1.0);   // |e| <= 2^-19: the seed sees the upper 32 bits of d2
+  const double t = fma(e, e, e);       // 1/(1 - e) = 1 + e + e^2 + O(e^3)
+  return fma(x, t, x);
 #else
   return 0.5 / d;
 #endif

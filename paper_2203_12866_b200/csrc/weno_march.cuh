@@ -50,8 +50,11 @@ struct MarchSmem {
 // March coordinates: cell j = 0..22 is tile row j (DIR > 0) or 23 - j (DIR < 0); interface m = 0..16 lies between cells
 // m + 3 and m + 4 and is biased towards smaller j (the upwind side); march row r' = 0..15 is cell r' + 4 and gets
 // F[r' + 1] - F[r'], stored at real row r' (DIR > 0) or 15 - r' (DIR < 0).  DIR == 0: per-lane direction (`neg`).
+// The first flux difference is stored after the second interface: only then must the flux-difference array of the slot be
+// free (barrier `bar_free`, phase parity `par_free`), so that wait hides behind the first two interfaces.
 template <int DIR>
-__device__ __forceinline__ void weno_march(uint32_t Ty0, uint32_t Tk0, bool neg, const cosenu_math::Weno7Beam& bm) {
+__device__ __forceinline__ void weno_march(uint32_t Ty0, uint32_t Tk0, bool neg, const cosenu_math::Weno7Beam& bm,
+                                           uint32_t bar_free, uint32_t par_free) {
   constexpr int RB = VC * 8;   // bytes per row
   uint32_t yb = Ty0, kb = Tk0;
   int ys = RB;
@@ -95,6 +98,7 @@ __device__ __forceinline__ void weno_march(uint32_t Ty0, uint32_t Tk0, bool neg,
   // NI - 1 - idx; whichever comes first (the upward march goes first within a step) forms it, once.
 #pragma unroll
   for (int s = 0; s < NLO; ++s) {
+    if (s == 1) mbar_wait(bar_free, par_free);
     {   // upward march, interface m = s: the new cell is m + 6
       const int m = s;
       if (2 * s + 6 <= NI - 1) c[m + 6] = cell(m + 6);
@@ -144,7 +148,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, 1)
   const int nchunks = (p.nv + VC - 1) / VC;
   const long long ntiles = (p.nz + TZ - 1) / TZ;
   const long long my_tiles = blockIdx.x < ntiles ? (ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
-  const long long nitems = my_tiles * nchunks;
+  const int nitems = (int)(my_tiles * nchunks);   // items of this CTA (fits: at most nz / 16 / gridDim.x * nv / 32)
   auto tile_of = [&](long long l) { const long long t = l + p.tile_shift; return t >= ntiles ? t - ntiles : t; };
 
   if (threadIdx.x == 0) {
@@ -161,7 +165,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, 1)
   if (warp >= MNW + MNC) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(MREG_DMA));
     if (warp == MNW + MNC && lane == 0) {
-      auto store_item = [&](long long m) {
+      auto store_item = [&](int m) {
         const int su = (int)(m & 1);
         const int iz0 = (int)(tile_of(blockIdx.x + (m / nchunks) * gridDim.x) * TZ), c0 = (int)(m % nchunks) * VC;
         mbar_wait(b_out_ready + 8 * su, (uint32_t)((m >> 1) & 1));
@@ -173,7 +177,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, 1)
       };
       long long ltile = blockIdx.x;
       int ch = 0;
-      for (long long n = 0; n < nitems; ++n) {
+      for (int n = 0; n < nitems; ++n) {
         const long long tile = tile_of(ltile);
         const int iz0 = (int)(tile * TZ);
         const int sy = (int)(n & 1), su = sy;
@@ -196,7 +200,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, 1)
         }
         if (++ch == nchunks) { ch = 0; ltile += gridDim.x; }
       }
-      for (long long m = nitems > 2 ? nitems - 2 : 0; m < nitems; ++m) store_item(m);
+      for (int m = nitems > 2 ? nitems - 2 : 0; m < nitems; ++m) store_item(m);
       tma_store_wait_all();
     }
     return;
@@ -206,7 +210,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, 1)
   if (warp < MNW) {
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(MREG_WENO));
     int ch = 0;
-    for (long long n = 0; n < nitems; ++n) {
+    for (int n = 0; n < nitems; ++n) {
       const int sy = (int)(n & 1), su = sy;
       const uint32_t par = (uint32_t)((n >> 1) & 1);
       const int j = ch * VC + lane;
@@ -216,10 +220,9 @@ __global__ void __launch_bounds__(MARCH_THREADS, 1)
       const uint32_t Ty0 = s_y + sy * SM::YTILE + (warp * ROWS * VC + lane) * 8;
       const uint32_t Tk0 = s_a + (su * 2 + 1) * SM::PTILE + (warp * TZ * VC + lane) * 8;
       mbar_wait(b_full_y + 8 * sy, par);
-      mbar_wait(b_a_free + 8 * su, par);
-      if (mpos == 0xffffffffu) weno_march<1>(Ty0, Tk0, false, bm);
-      else if (mpos == 0u) weno_march<-1>(Ty0, Tk0, true, bm);
-      else weno_march<0>(Ty0, Tk0, v < 0.0, bm);
+      if (mpos == 0xffffffffu) weno_march<1>(Ty0, Tk0, false, bm, b_a_free + 8 * su, par);
+      else if (mpos == 0u) weno_march<-1>(Ty0, Tk0, true, bm, b_a_free + 8 * su, par);
+      else weno_march<0>(Ty0, Tk0, v < 0.0, bm, b_a_free + 8 * su, par);
       __syncwarp();
       if (lane == 0) {
         mbar_arrive(b_empty_y + 8 * sy);
@@ -247,7 +250,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, 1)
   double min_cur = 0.0, min_next = load_min(blockIdx.x);
   long long ltile = blockIdx.x;
   int ch = 0;
-  for (long long n = 0; n < nitems; ++n) {
+  for (int n = 0; n < nitems; ++n) {
     const long long iz0 = tile_of(ltile) * TZ;
     if (ch == 0) {
       min_cur = p.mu * min_next;
@@ -268,6 +271,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, 1)
     mbar_wait(b_k_ready + 8 * su, par);
     mbar_wait(b_full_y + 8 * sy, par);    // already complete (the WENO warps have consumed the slot): orders my reads after the TMA writes
     mbar_wait(b_full_a + 8 * su, par);
+    double ycl[8];
 #pragma unroll
     for (int s = 0; s < MRC; ++s) {
       const int row = row0 + s;
@@ -275,11 +279,21 @@ __global__ void __launch_bounds__(MARCH_THREADS, 1)
       const bool act = active && (iz < p.nz);
       const int tr = row + H;
       double yc[8], k[8];
+      if (s < MRC - 2) {
 #pragma unroll
-      for (int c = 0; c < 8; ++c) yc[c] = lds(Ty + ((c * ROWS + tr) * VC) * 8);
-      if (s == MRC - 1) {   // the stage-input slot is no longer needed by this warp
+        for (int c = 0; c < 8; ++c) yc[c] = lds(Ty + ((c * ROWS + tr) * VC) * 8);
+      } else if (s == MRC - 2) {
+        // the cell values of the last two rows are read together, so that the stage-input slot is released half way
+        // through the combine step (the TMA load of the item after next waits for it)
+#pragma unroll
+        for (int c = 0; c < 8; ++c) yc[c] = lds(Ty + ((c * ROWS + tr) * VC) * 8);
+#pragma unroll
+        for (int c = 0; c < 8; ++c) ycl[c] = lds(Ty + ((c * ROWS + tr + 1) * VC) * 8);
         __syncwarp();
         if (lane == 0) mbar_arrive(b_empty_y + 8 * sy);
+      } else {
+#pragma unroll
+        for (int c = 0; c < 8; ++c) yc[c] = ycl[c];
       }
       // ---- S3: Hamiltonian from the moments (mu folded in), commutator
       {
