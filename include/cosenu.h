@@ -50,7 +50,8 @@ enum { COSENU_OK = 0, COSENU_EINVAL = 1, COSENU_ENOMEM = 2, COSENU_ECUDA = 3, CO
 /* option keys of cosenu_set_option */
 enum {
   COSENU_OPT_EPS_KO = 0,   /* Kreiss-Oliger strength eps_KO of Eq. (5); default 0.1; >= 0 */
-  COSENU_OPT_WENO_EPS = 1, /* epsilon of Eq. (14); default 1e-6; 0 < eps <= 1e30 */
+  COSENU_OPT_WENO_EPS = 1, /* epsilon of Eq. (14); default 1e-6; 1e-40 <= eps <= 1e30 (the range the
+                              one-division form of the weights supports on every beam, v = 0 included) */
   COSENU_OPT_ADVECT = 2,   /* 0 switches the advection term off (commutator-only runs); default 1 */
   COSENU_OPT_RK_FORM = 3,  /* how the classical RK4 combination is carried between the 4 stage launches
                               (same method, same result up to rounding; differs in HBM traffic per cell-step):
@@ -72,6 +73,9 @@ enum {
                               handle's own launches, which removes the per-launch host cost on the small, launch-bound grids;
                               0: always launch kernel by kernel.  Not used on slab handles (their launch parameters change every
                               stage) nor while COSENU_OPT_STAGE_TIMING is on. */
+  COSENU_OPT_MAX_CTAS = 9, /* cap of the persistent grid of a stage launch (0, default: one CTA per SM).  With a cap of at most half the SMs
+                              the stage kernels of two slab handles driven from two streams are co-resident, which is how the fused
+                              halo exchange is exercised on one GPU (tests/test_gpu_slab.py); no other use */
   COSENU_OPT_KO_ORDER = 7, /* r of the Kreiss-Oliger operator of Eq. (5): 2 (default; "r = 2 for most numerical
                               experiments"; 5-point, halo 2) or 3 (7-point (eps/64dz) delta^6, halo 3).  FD scheme only;
                               the handle's stream is idle when this is changed. */

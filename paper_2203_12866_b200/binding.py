@@ -15,6 +15,7 @@ LIB_PATH = os.path.join(HERE, "libcosenu_b200.so")
 FD4_KO3, FV_WENO7 = 0, 1
 OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, 1, 2, 3, 4
 OPT_EPS_KO, OPT_WENO_EPS, OPT_ADVECT, OPT_RK_FORM, OPT_STAGE_TIMING, OPT_VARIANT, OPT_QUADRATURE, OPT_KO_ORDER, OPT_GRAPH = 0, 1, 2, 3, 4, 5, 6, 7, 8
+OPT_MAX_CTAS = 9
 
 # every symbol include/cosenu.h declares
 SYMBOLS = ["cosenu_create", "cosenu_workspace_bytes", "cosenu_attach", "cosenu_set_option", "cosenu_init",

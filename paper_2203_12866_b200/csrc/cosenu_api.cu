@@ -52,6 +52,7 @@ struct cosenu {
   int device = 0;
   int variant = 0;       // kernel shape variant (COSENU_OPT_VARIANT)
   int num_sms = 148;
+  int max_ctas = 0;      // COSENU_OPT_MAX_CTAS: cap of the persistent grid of a stage launch (0: one CTA per SM)
 
   // workspace
   void* ws = nullptr; size_t ws_bytes = 0; bool ws_owned = false;
@@ -108,11 +109,31 @@ int fail(cosenu* h, int code, const std::string& msg) {
 int cuda_fail(cosenu* h, cudaError_t e, const char* what) {
   return fail(h, COSENU_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
 }
+// every entry point that touches CUDA runs on the handle's device and leaves the caller's current device as it found it
+struct DeviceGuard {
+  int prev = -1; bool changed = false;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) changed = cudaSetDevice(dev) == cudaSuccess;
+  }
+  ~DeviceGuard() { if (changed) cudaSetDevice(prev); }
+  DeviceGuard(const DeviceGuard&) = delete;
+  DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
 #define CK(call)                                                  \
   do {                                                            \
     cudaError_t e_ = (call);                                      \
     if (e_ != cudaSuccess) return cuda_fail(h, e_, #call);        \
   } while (0)
+
+// z-slab: a halo wait that gave up (a neighbour that never delivered its rows) leaves stale ghost rows behind: every call
+// that hands results to the caller reports it.  The stream is idle here (the callers have just synchronised it).
+int halo_check(cosenu* h, const char* who) {
+  if (!h->slab || !h->maps_ready) return COSENU_OK;
+  int v = 0;
+  CK(cudaMemcpy(&v, h->d_err, sizeof(int), cudaMemcpyDeviceToHost));
+  if (v) return fail(h, COSENU_ESTATE, std::string(who) + ": a halo wait timed out (a neighbouring slab never delivered its ghost rows); the state is invalid");
+  return COSENU_OK;
+}
 
 size_t workspace_layout(const cosenu* h, size_t off[11]) {
   const size_t st = align_up(sizeof(double) * 8 * (size_t)(h->nz + 2 * G) * h->nvp, 256);
@@ -203,6 +224,13 @@ int make_maps(cosenu* h) {
   return COSENU_OK;
 }
 
+// persistent grid of a stage launch: one CTA per SM, fewer when there are fewer tiles or the caller caps it (COSENU_OPT_MAX_CTAS)
+unsigned grid_size(const cosenu* h, long long ntiles) {
+  long long g = ntiles < h->num_sms ? ntiles : h->num_sms;
+  if (h->max_ctas > 0 && g > h->max_ctas) g = h->max_ctas;
+  return (unsigned)g;
+}
+
 template <int SCHEME, int KIND, int TZ, int NSEG, int NY, int NUA>
 int launch_one(cosenu* h, int in_buf, int out_buf, int a1_buf, int a2_buf, const StageParams& p0) {
   constexpr int T = TZ == TZ_ALL ? 0 : (TZ == TZ_WENO1 ? 1 : (TZ == TZ_WENO2 ? 2 : 3));
@@ -218,7 +246,7 @@ int launch_one(cosenu* h, int in_buf, int out_buf, int a1_buf, int a2_buf, const
   }
   if (h->dry_run) return COSENU_OK;
   const long long ntiles = (h->nz + TZ - 1) / TZ;
-  const unsigned grid = (unsigned)(ntiles < h->num_sms ? ntiles : h->num_sms);   // persistent: one CTA per SM
+  const unsigned grid = grid_size(h, ntiles);   // persistent: one CTA per SM
   StageParams p = p0;
   if (h->slab) p.tile_shift = ntiles >= 3 ? ntiles - 2 : 0;   // walk the (up to two) high edge tiles, then tile 0, first
   kern<<<grid, NSEG * 32 + 32, smem, h->stream>>>(map, h->tp[T][0], a1, a2, omap, p);
@@ -240,7 +268,7 @@ int launch_march(cosenu* h, int in_buf, int out_buf, int acc_buf, const StagePar
   }
   if (h->dry_run) return COSENU_OK;
   const long long ntiles = (h->nz + MTZ - 1) / MTZ;
-  const unsigned grid = (unsigned)(ntiles < h->num_sms ? ntiles : h->num_sms);   // persistent: one CTA per SM
+  const unsigned grid = grid_size(h, ntiles);   // persistent: one CTA per SM
   StageParams p = p0;
   if (h->slab) p.tile_shift = ntiles >= 3 ? ntiles - 2 : 0;
   kern<<<grid, MARCH_THREADS, smem, h->stream>>>(h->tm[0][in_buf], h->tp[0][0], h->tp[0][acc_buf], h->tp[0][out_buf], p);
@@ -627,9 +655,16 @@ extern "C" size_t cosenu_workspace_bytes(const cosenu_t* h) {
 extern "C" int cosenu_attach(cosenu_t* h, void* dev_workspace, size_t bytes, void* cuda_stream) {
   if (!h) return COSENU_EINVAL;
   if (h->maps_ready) return fail(h, COSENU_ESTATE, "cosenu_attach: workspace already in use");
+  DeviceGuard dg_(h->device);
   if (dev_workspace) {
     if (bytes < cosenu_workspace_bytes(h) || (reinterpret_cast<uintptr_t>(dev_workspace) & 255))
       return fail(h, COSENU_EINVAL, "cosenu_attach: workspace too small or not 256-byte aligned");
+    // the kernels and the TMA descriptors need plain device memory of the handle's device
+    cudaPointerAttributes at;
+    cudaError_t e = cudaPointerGetAttributes(&at, dev_workspace);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return cuda_fail(h, e, "cosenu_attach: cudaPointerGetAttributes"); }
+    if (at.type != cudaMemoryTypeDevice || at.device != h->device)
+      return fail(h, COSENU_EINVAL, "cosenu_attach: the workspace is not device memory of the device the handle was created on");
     h->ws = dev_workspace; h->ws_bytes = bytes; h->ws_owned = false;
   }
   h->stream = static_cast<cudaStream_t>(cuda_stream);
@@ -638,11 +673,13 @@ extern "C" int cosenu_attach(cosenu_t* h, void* dev_workspace, size_t bytes, voi
 
 extern "C" int cosenu_set_option(cosenu_t* h, int key, double value) {
   if (!h) return COSENU_EINVAL;
+  DeviceGuard dg_(h->device);
   drop_graph(h);   // the captured launch parameters may change
   switch (key) {
     case COSENU_OPT_GRAPH: h->use_graph = value != 0; return COSENU_OK;
     case COSENU_OPT_EPS_KO: if (!(value >= 0) || !std::isfinite(value)) break; h->eps_ko = value; return COSENU_OK;
-    case COSENU_OPT_WENO_EPS: if (!(value > 0) || !(value <= 1e30)) break; h->weno_eps = value; return COSENU_OK;
+    case COSENU_OPT_WENO_EPS: if (!(value >= 1e-40) || !(value <= 1e30)) break; h->weno_eps = value; return COSENU_OK;   // range of the product form, weno7_math.h
+    case COSENU_OPT_MAX_CTAS: if (!(value >= 0) || !(value <= 65535) || value != std::floor(value)) break; h->max_ctas = (int)value; return COSENU_OK;
     case COSENU_OPT_ADVECT: h->advect = value != 0; return COSENU_OK;
     case COSENU_OPT_RK_FORM: if (value != 0 && value != 1 && value != 2 && value != 3) break; h->rk_form = (int)value; return COSENU_OK;
     case COSENU_OPT_VARIANT: if (value != 0 && value != 1 && value != 2 && value != 3 && value != 4) break; h->variant = (int)value; return COSENU_OK;
@@ -674,6 +711,7 @@ extern "C" int cosenu_set_option(cosenu_t* h, int key, double value) {
 
 extern "C" int cosenu_set_state(cosenu_t* h, const double* host_state, double t) {
   if (!h || !host_state || !std::isfinite(t)) return h ? fail(h, COSENU_EINVAL, "cosenu_set_state: invalid argument") : COSENU_EINVAL;
+  DeviceGuard dg_(h->device);
   int rc = ensure_workspace(h);
   if (rc) return rc;
   for (int c = 0; c < 8; ++c) {
@@ -749,7 +787,7 @@ extern "C" int cosenu_step(cosenu_t* h, int64_t n) {
   if (h->slab && !(h->linked && h->ghosts_pushed))
     return fail(h, COSENU_ESTATE, "cosenu_step: a slab must be linked (cosenu_slab_link) and its ghost rows exchanged "
                                   "(cosenu_slab_push_ghosts) first");
-  CK(cudaSetDevice(h->device));
+  DeviceGuard dg_(h->device);
   if (h->use_graph && !h->slab && !h->stage_timing && n >= 2 * GRAPH_STEPS) {
     if (!h->gexec && build_graph(h) != COSENU_OK) {
       // capture not possible here (e.g. a caller stream that is itself being captured): launch kernel by kernel from now on
@@ -772,25 +810,28 @@ extern "C" int cosenu_step(cosenu_t* h, int64_t n) {
 
 extern "C" int cosenu_sync(cosenu_t* h) {
   if (!h) return COSENU_EINVAL;
+  DeviceGuard dg_(h->device);
   CK(cudaStreamSynchronize(h->stream));
-  return COSENU_OK;
+  return halo_check(h, "cosenu_sync");
 }
 
 extern "C" int cosenu_get_state(cosenu_t* h, double* host_out) {
   if (!h || !host_out) return COSENU_EINVAL;
   if (!h->have_state) return fail(h, COSENU_ESTATE, "cosenu_get_state: no state");
+  DeviceGuard dg_(h->device);
   for (int c = 0; c < 8; ++c) {
     CK(cudaMemcpy2DAsync(host_out + (size_t)c * h->nz * h->nv, sizeof(double) * h->nv,
                          h->U + c * h->comp_stride + (size_t)G * h->nvp, sizeof(double) * h->nvp, sizeof(double) * h->nv,
                          (size_t)h->nz, cudaMemcpyDeviceToHost, h->stream));
   }
   CK(cudaStreamSynchronize(h->stream));
-  return COSENU_OK;
+  return halo_check(h, "cosenu_get_state");
 }
 
 extern "C" int cosenu_get_moments(cosenu_t* h, double* host_out) {
   if (!h || !host_out) return COSENU_EINVAL;
   if (!h->have_state) return fail(h, COSENU_ESTATE, "cosenu_get_moments: no state");
+  DeviceGuard dg_(h->device);
   CK(cudaMemcpyAsync(host_out, h->M[h->mcur], sizeof(double) * 6 * (size_t)h->nz, cudaMemcpyDeviceToHost, h->stream));
   CK(cudaStreamSynchronize(h->stream));
   return COSENU_OK;
@@ -801,6 +842,7 @@ extern "C" int cosenu_diagnostics(cosenu_t* h, cosenu_diag_t* d) {
   if (!h->have_state) return fail(h, COSENU_ESTATE, "cosenu_diagnostics: no state");
   if (h->slab) return fail(h, COSENU_ESTATE, "cosenu_diagnostics: a slab holds part of the grid; use cosenu_slab_diag_sums + "
                                              "a reduction over the slabs + cosenu_slab_diag_finish");
+  DeviceGuard dg_(h->device);
   double g[DIAG_NVAL];
   int rc = diag_sums(h, g);
   if (rc) return rc;
@@ -812,6 +854,7 @@ extern "C" int64_t cosenu_launch_count(const cosenu_t* h) { return h ? h->launch
 
 extern "C" int cosenu_stage_times(cosenu_t* h, double* ms_sum, int64_t* launches_per_stage) {
   if (!h || !ms_sum || !launches_per_stage) return COSENU_EINVAL;
+  DeviceGuard dg_(h->device);
   int rc = drain_events(h);
   if (rc) return rc;
   for (int k = 0; k < 4; ++k) { ms_sum[k] = h->stage_ms[k]; h->stage_ms[k] = 0; }
@@ -821,7 +864,7 @@ extern "C" int cosenu_stage_times(cosenu_t* h, double* ms_sum, int64_t* launches
 
 extern "C" void cosenu_destroy(cosenu_t* h) {
   if (!h) return;
-  cudaSetDevice(h->device);
+  DeviceGuard dg_(h->device);
   if (h->maps_ready) cudaStreamSynchronize(h->stream);
   for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
   drop_graph(h);
@@ -842,6 +885,7 @@ typedef CUresult (*PFN_getAddressRange)(CUdeviceptr*, size_t*, CUdeviceptr);
 extern "C" int cosenu_slab_export(cosenu_t* h, cosenu_slab_peer_t* out) {
   if (!h || !out) return COSENU_EINVAL;
   if (!h->slab) return fail(h, COSENU_ESTATE, "cosenu_slab_export: not a slab handle (cosenu_create_slab)");
+  DeviceGuard dg_(h->device);
   int rc = ensure_workspace(h);
   if (rc) return rc;
   CK(cudaStreamSynchronize(h->stream));   // the workspace is zeroed (counters start at 0) before anybody can reach it
@@ -880,6 +924,7 @@ extern "C" int cosenu_slab_link(cosenu_t* h, const cosenu_slab_peer_t* lo, const
   if (!h || !lo || !hi) return COSENU_EINVAL;
   if (!h->slab) return fail(h, COSENU_ESTATE, "cosenu_slab_link: not a slab handle");
   if (h->linked) return fail(h, COSENU_ESTATE, "cosenu_slab_link: already linked");
+  DeviceGuard dg_(h->device);   // peer access is enabled FROM the current device, IPC handles are opened on it
   int rc = ensure_workspace(h);
   if (rc) return rc;
   const cosenu_slab_peer_t* peers[2] = {lo, hi};
@@ -921,7 +966,7 @@ extern "C" int cosenu_slab_push_ghosts(cosenu_t* h) {
   if (!h) return COSENU_EINVAL;
   if (!h->slab || !h->linked) return fail(h, COSENU_ESTATE, "cosenu_slab_push_ghosts: slab not linked");
   if (!h->have_state) return fail(h, COSENU_ESTATE, "cosenu_slab_push_ghosts: no state");
-  CK(cudaSetDevice(h->device));
+  DeviceGuard dg_(h->device);
   push_ghosts_kernel<<<64, 256, 0, h->stream>>>(h->U, h->nz, h->nvp, h->comp_stride, G,
                                                 h->peer_buf[0][0] + (size_t)(h->peer_nz[0] + G) * h->nvp, h->peer_stride[0],
                                                 h->peer_buf[1][0], h->peer_stride[1]);
@@ -935,19 +980,23 @@ extern "C" int cosenu_slab_push_ghosts(cosenu_t* h) {
 extern "C" int cosenu_slab_ref_sums(cosenu_t* h, double* out) {
   if (!h || !out) return COSENU_EINVAL;
   if (!h->have_state) return fail(h, COSENU_ESTATE, "cosenu_slab_ref_sums: no state");
+  DeviceGuard dg_(h->device);
   return ref_sums(h, out);
 }
 
 extern "C" int cosenu_slab_set_ref_sums(cosenu_t* h, const double* global_sums) {
   if (!h || !global_sums) return COSENU_EINVAL;
   if (!h->have_state) return fail(h, COSENU_ESTATE, "cosenu_slab_set_ref_sums: no state");
+  DeviceGuard dg_(h->device);
   return set_ref_sums(h, global_sums);
 }
 
 extern "C" int cosenu_slab_diag_sums(cosenu_t* h, double* out10) {
   if (!h || !out10) return COSENU_EINVAL;
   if (!h->have_state) return fail(h, COSENU_ESTATE, "cosenu_slab_diag_sums: no state");
-  return diag_sums(h, out10);
+  DeviceGuard dg_(h->device);
+  int rc = diag_sums(h, out10);
+  return rc ? rc : halo_check(h, "cosenu_slab_diag_sums");
 }
 
 extern "C" int cosenu_slab_diag_finish(cosenu_t* h, const double* global10, int set_reference, cosenu_diag_t* out) {
@@ -967,8 +1016,7 @@ extern "C" int cosenu_slab_step_group(cosenu_t** hs, int32_t count, int64_t n) {
     if (h->stream != hs[0]->stream || h->device != hs[0]->device)
       return fail(h, COSENU_EINVAL, "cosenu_slab_step_group: the slabs of a group share one device and one stream");
   }
-  cudaError_t e = cudaSetDevice(hs[0]->device);
-  if (e != cudaSuccess) return cuda_fail(hs[0], e, "cudaSetDevice");
+  DeviceGuard dg_(hs[0]->device);
   for (int64_t s = 0; s < n; ++s) {
     for (int k = 0; k < 4; ++k)
       for (int i = 0; i < count; ++i) {
@@ -984,7 +1032,7 @@ extern "C" int cosenu_slab_stage(cosenu_t* h, int32_t k) {
   if (!h || k < 0 || k > 3) return h ? fail(h, COSENU_EINVAL, "cosenu_slab_stage: k must be 0..3") : COSENU_EINVAL;
   if (!h->slab || !h->linked || !h->ghosts_pushed || !h->have_state)
     return fail(h, COSENU_ESTATE, "cosenu_slab_stage: the slab must be linked, hold a state and have its ghosts exchanged");
-  CK(cudaSetDevice(h->device));
+  DeviceGuard dg_(h->device);
   int rc = rk_stage(h, k);
   if (rc) return rc;
   if (k == 3) { h->t += h->dt; h->step += 1; }
@@ -994,6 +1042,7 @@ extern "C" int cosenu_slab_stage(cosenu_t* h, int32_t k) {
 extern "C" int cosenu_slab_wait_failed(cosenu_t* h, int32_t* failed) {
   if (!h || !failed) return COSENU_EINVAL;
   if (!h->maps_ready) { *failed = 0; return COSENU_OK; }
+  DeviceGuard dg_(h->device);
   int v = 0;
   CK(cudaMemcpyAsync(&v, h->d_err, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
   CK(cudaStreamSynchronize(h->stream));

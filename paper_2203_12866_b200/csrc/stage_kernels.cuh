@@ -107,8 +107,6 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "r"(parity)
       : "memory");
 }
-// the DMA warp's wait: same, kept separate so that the profile shows which side waits
-__device__ __forceinline__ void mbar_wait_backoff(uint32_t bar, uint32_t parity) { mbar_wait(bar, parity); }
 // 3-D tiled TMA load global -> shared, completion on an mbarrier
 __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1, int c2) {
   asm volatile(
@@ -153,6 +151,7 @@ __device__ __forceinline__ unsigned long long global_timer_ns() {
 // wait until *ctr >= val; gives up after ~4 s (sets *err) so that a missing neighbour is an error, not a hang
 __device__ __noinline__ void wait_arrivals(const unsigned long long* ctr, unsigned long long val, int* err) {
   if (ld_acquire_sys(ctr) >= val) return;
+  if (err && *reinterpret_cast<volatile int*>(err)) return;   // an earlier wait has already given up: the run is invalid, do not add 4 s per tile
   const unsigned long long t0 = global_timer_ns();
   while (ld_acquire_sys(ctr) < val) {
     __nanosleep(200);
@@ -345,7 +344,7 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
       auto store_item = [&](long long m) {   // outputs of item m
         const int su = (int)(m % NUA);
         const int iz0 = (int)(tile_of(blockIdx.x + (m / nchunks) * gridDim.x) * TZ), c0 = (int)(m % nchunks) * VC;
-        mbar_wait_backoff(b_out_ready + 8 * su, (uint32_t)((m / NUA) & 1));
+        mbar_wait(b_out_ready + 8 * su, (uint32_t)((m / NUA) & 1));
         const uint32_t src = s_ua + su * NARR * SM::PTILE;
         tma_store_3d(&tm_out, src, c0, iz0, 0);
         if constexpr (KT::WRITE_ACC) tma_store_3d(&tm_acc, src + SM::PTILE, c0, iz0, 0);
@@ -366,7 +365,7 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
           if (p.wait_hi != nullptr && (tile + 1) * TZ + G > p.nz) { wait_arrivals(p.wait_hi, p.wait_val, p.err_flag); waited = true; }
           if (waited) asm volatile("fence.proxy.async.global;" ::: "memory");   // generic-proxy acquire -> TMA (async proxy) reads
         }
-        mbar_wait_backoff(b_empty_y + 8 * sy, (uint32_t)(((n / NY) & 1) ^ 1));
+        mbar_wait(b_empty_y + 8 * sy, (uint32_t)(((n / NY) & 1) ^ 1));
         mbar_expect_tx(b_full_y + 8 * sy, SM::YTILE);
         tma_load_3d(s_y + sy * SM::YTILE, &tm_y, b_full_y + 8 * sy, ch * VC, iz0 + G - H, 0);
         if (n >= NUA) store_item(n - NUA);

@@ -31,8 +31,8 @@
 //      P_r  = prod_{m != r} qs_m^2,
 //      F = sum_r w_r fhat_r / sum_r w_r = u_i + (1/2) [sum_r P_r (A_r + s_r/6)] / [sum_r P_r].
 // The per-beam constants  eps_r = (eps/v^2)/sqrt(d_r)  are formed once per beam (Weno7Beam).
-// Range: needs |u|^2 * 1e4 / v^2-scaled terms to stay below ~1e50 per factor (states are O(1)); v^2 is
-// clamped to >= 1e-40 (the flux is multiplied by v afterwards, so v = 0 gives exactly 0).
+// Range: needs |u|^2 * 1e4 / v^2-scaled terms to stay below ~1e50 per factor (states are O(1)); eps / v^2 is
+// clamped to <= 1e45 (the flux is multiplied by v afterwards, so v = 0 gives exactly 0); 1e-40 <= eps <= 1e30.
 #ifndef COSENU_WENO7_MATH_H
 #define COSENU_WENO7_MATH_H
 
@@ -68,9 +68,11 @@ struct Weno7Beam {
   double e0, e1, e2, e3;
 };
 COSENU_HD Weno7Beam weno7_beam(double v, double eps) {
-  double v2 = v * v;
-  if (v2 < 1e-40) v2 = 1e-40;
-  const double ev = eps / v2;
+  // eps / v^2, kept below 1e45 so that the products of six q_r stay in range for every accepted eps (1e-40 .. 1e30), also
+  // on a beam with v = 0 exactly (vertex-centred grids); there the flux is multiplied by |v| = 0 afterwards
+  const double v2 = v * v;
+  double ev = eps / (v2 < 1e-300 ? 1e-300 : v2);
+  if (ev > 1e45) ev = 1e45;
   Weno7Beam b;
   b.e0 = ev * 2.9580398915498080213;   // sqrt(35/4)
   b.e1 = ev * 1.3944333775567926;      // sqrt(35/18)

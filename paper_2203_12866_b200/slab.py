@@ -177,9 +177,10 @@ class CosenuSlab:
                 self.ring.barrier()
 
     def sync(self):
-        self.sim.sync()
-        if _wait_failed(self.sim):
-            raise B.CosenuError(B.ECUDA, "a halo wait timed out: a neighbouring slab did not deliver its edge rows")
+        self.sim.sync()        # raises if a halo wait of this slab gave up (cosenu_sync checks the flag)
+
+    def wait_failed(self):
+        return _wait_failed(self.sim)
 
     def get_state(self, out=None):
         return self.sim.get_state(out)
@@ -255,9 +256,7 @@ class SlabGroup:
 
     def sync(self):
         for s in self.sims:
-            s.sync()
-            if _wait_failed(s):
-                raise B.CosenuError(B.ECUDA, "a halo wait timed out")
+            s.sync()           # raises if a halo wait of that slab gave up
 
     def get_state(self):
         return np.concatenate([s.get_state() for s in self.sims], axis=1)
@@ -278,3 +277,51 @@ class SlabGroup:
         for s in self.sims:
             s.close()
         self.sims = []
+
+
+class ConcurrentSlabs(SlabGroup):
+    """`nslabs` slabs of one periodic grid in ONE process on ONE device, every slab on a stream of its OWN and driven by a host
+    thread of its own with the free-running `cosenu_step(n)`: no host synchronisation between the stages, nothing orders the
+    slabs' launches but the arrival counters in device memory.  With `max_ctas` <= (SMs / nslabs) the stage kernels of all
+    slabs are co-resident (one CTA per SM each), so the kernels really spin on each other: this is the halo-exchange
+    protocol of a multi-GPU run (RAW wait, WAR argument of DESIGN.md section 8) on one GPU.
+    """
+
+    def __init__(self, nslabs, nz_global, nv, L, dt, omega, theta, mu, scheme, max_ctas, bounds=None, **opts):
+        import torch
+        self.nz_global, self.nv = int(nz_global), int(nv)
+        self.bounds = bounds if bounds is not None else [slab_bounds(nz_global, nslabs, r) for r in range(nslabs)]
+        self._streams = [torch.cuda.Stream() for _ in self.bounds]
+        self.sims = [B.Cosenu(nzl, nv, L, dt, omega, theta, mu, scheme, use_torch_workspace=False, stream=st,
+                              slab=(nz_global, zb), **opts) for (zb, nzl), st in zip(self.bounds, self._streams)]
+        for s in self.sims:
+            s.set_option(B.OPT_MAX_CTAS, max_ctas)
+        peers = [_export(s) for s in self.sims]
+        n = len(self.sims)
+        for r, s in enumerate(self.sims):
+            lo, hi = neighbours(n, r)
+            _link(s, peers[lo], peers[hi])
+        self._L = self.sims[0]._L
+
+    def step(self, n=1, delays=None):
+        """Every slab's thread enqueues its n steps (4 n launches) on its own stream; delays[r] seconds of head start skew."""
+        import threading
+        import time
+        errs = [None] * len(self.sims)
+
+        def run(r):
+            try:
+                if delays and delays[r]:
+                    time.sleep(delays[r])
+                self.sims[r].step(n)
+            except Exception as e:   # noqa: BLE001  (reported to the caller below)
+                errs[r] = e
+
+        th = [threading.Thread(target=run, args=(r,)) for r in range(len(self.sims))]
+        for t in th:
+            t.start()
+        for t in th:
+            t.join()
+        for e in errs:
+            if e is not None:
+                raise e

@@ -392,3 +392,57 @@ def test_full_size_cfg4_windows(B, R):
     assert d["trace_dev_max"] <= 1e-12
     s2, c2 = np.sin(2 * c["theta"]), np.cos(2 * c["theta"])
     assert abs(s2 * d["dM0"][0] - c2 * d["dM0"][2]) <= 1e-9 * c["nz"]
+
+
+@pytest.mark.parametrize("variant", [0, 3])
+@pytest.mark.parametrize("eps", [1e-30, 1e-6, 1e10, 1e30])
+def test_weno_eps_range_with_a_v0_beam(B, R, eps, variant):
+    """Simpson grid with nv odd: the beam j = (nv - 1)/2 has v = 0 exactly.  Every accepted epsilon of Eq. (14) gives finite
+    results there (eps / v^2 is clamped inside the product form of the weights, csrc/weno7_math.h) and agrees with the oracle."""
+    nz, nv = 200, 17
+    st = inputs.random_state(nz, nv, seed=611)
+    args = (nz, nv, 0.7 * nz, 0.05, 0.8, 0.3, 1.3, FV)
+    got, ref, gm, rm, _, _ = run_pair(B, R, args, st, 2, quadrature=2, weno_eps=eps, variant=variant)
+    assert np.all(np.isfinite(got))
+    assert np.max(np.abs(got - ref)) <= 1e-12 * max(1.0, np.max(np.abs(ref)))
+    assert np.max(np.abs(gm - rm)) <= 1e-12 * max(1.0, np.max(np.abs(rm)))
+
+
+def test_option_ranges_and_attach_validation(B):
+    import ctypes as C
+    g = B.Cosenu(64, 16, 64.0, 0.1, 0, 0, 1.0, FV)
+    for bad in (0.0, 1e-50, 1e31, float("nan")):
+        with pytest.raises(B.CosenuError):
+            g.set_option(B.OPT_WENO_EPS, bad)
+    for bad in (-1, 0.5, 1e9):
+        with pytest.raises(B.CosenuError):
+            g.set_option(B.OPT_MAX_CTAS, bad)
+    g.set_option(B.OPT_MAX_CTAS, 3)
+    g.set_option(B.OPT_MAX_CTAS, 0)
+    g.close()
+    # a workspace that is not device memory is refused (the kernels and the TMA descriptors need device memory)
+    L = B.load()
+    h = L.cosenu_create(64, 16, 64.0, 0.1, 0.0, 0.0, 1.0, FV)
+    assert h
+    need = L.cosenu_workspace_bytes(h)
+    host = np.zeros(need // 8 + 64, dtype=np.float64)
+    addr = (host.ctypes.data + 255) // 256 * 256
+    assert L.cosenu_attach(h, C.c_void_p(addr), need, None) != 0
+    L.cosenu_destroy(h)
+
+
+def test_capped_grid_is_bitwise_identical(B):
+    """COSENU_OPT_MAX_CTAS only changes which CTA walks which tile."""
+    nz, nv = 16 * 40, 48
+    st = inputs.random_state(nz, nv, seed=9)
+    for scheme in (FD, FV):
+        outs = []
+        for cap in (0, 7):
+            g = B.Cosenu(nz, nv, 0.7 * nz, 0.05, 0.8, 0.3, 1.3, scheme)
+            if cap:
+                g.set_option(B.OPT_MAX_CTAS, cap)
+            g.set_state(st)
+            g.step(3)
+            outs.append((g.get_state(), g.get_moments()))
+            g.close()
+        assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])

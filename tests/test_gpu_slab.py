@@ -199,3 +199,77 @@ def test_slabs_in_separate_processes_over_cuda_ipc(B, scheme, world):
     assert np.array_equal(got, ref)
     for o in outs:
         assert abs(o[4]["psurv_nu"] - refd["psurv_nu"]) <= 1e-13 and o[4]["step"] == nsteps
+
+
+# ------------------------------------------------------------------ the halo-exchange protocol under real concurrency
+def _sm_count():
+    import torch
+    return torch.cuda.get_device_properties(0).multi_processor_count
+
+
+@pytest.mark.parametrize("scheme", [FD, FV])
+@pytest.mark.parametrize("nslabs,skew", [(2, None), (2, (0.0, 0.3)), (2, (0.3, 0.0)), (3, None), (3, (0.2, 0.0, 0.1))])
+def test_free_running_slabs_spin_on_each_other(B, S, scheme, nslabs, skew):
+    """Every slab on its own stream, driven by its own host thread with the free-running cosenu_step(n); the persistent grid
+    of every stage launch is capped (COSENU_OPT_MAX_CTAS) so that the kernels of all slabs are co-resident (one CTA per SM
+    each) and nothing but the arrival counters orders them: the RAW wait and the WAR argument of DESIGN.md section 8 with
+    kernels that really wait for each other -- also when one rank starts late.  Bit-identical to the single domain."""
+    cap = _sm_count() // nslabs
+    tiles_per_cta = 2
+    nz = nslabs * cap * 16 * tiles_per_cta + (16 * 3 if nslabs == 3 else 0)     # every slab fills its capped grid; 3 slabs: ragged
+    nv = 64
+    st = inputs.random_state(nz, nv, seed=900 + nslabs)
+    args = (nz, nv, 0.7 * nz, 0.05, 0.8, 0.3, 1.3, scheme)
+    ref, refm, _ = _single(B, args, st, 12)
+    grp = S.ConcurrentSlabs(nslabs, *args, max_ctas=cap)
+    grp.set_state(st)
+    grp.step(12, delays=skew)
+    grp.sync()                       # raises if any halo wait timed out
+    got, gotm = grp.get_state(), grp.get_moments()
+    grp.close()
+    assert np.array_equal(got, ref)
+    assert np.array_equal(gotm, refm)
+
+
+def test_missing_neighbour_is_an_error_not_a_hang(B, S):
+    """One slab of two steps alone: its waits give up, the flag is raised, and every call that hands results out reports it."""
+    nz, nv = 2 * 16 * 8, 32
+    st = inputs.random_state(nz, nv, seed=77)
+    grp = S.ConcurrentSlabs(2, nz, nv, 0.7 * nz, 0.05, 0.8, 0.3, 1.3, FV, max_ctas=8)
+    grp.set_state(st)
+    grp.sims[0].step(1)              # slab 1 never steps: stage 2 of slab 0 waits for rows that never come
+    with pytest.raises(B.CosenuError):
+        grp.sims[0].sync()
+    assert S._wait_failed(grp.sims[0])
+    with pytest.raises(B.CosenuError):
+        grp.sims[0].get_state()
+    for s in grp.sims:
+        s.close()
+    grp.sims = []
+
+
+def test_two_gpus_free_running(B, S):
+    """Two slabs on two GPUs of this process (peer access), free-running: needs a box with at least two devices."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two CUDA devices")
+    nz, nv = 2 * 148 * 16, 64
+    st = inputs.random_state(nz, nv, seed=31)
+    args = (nz, nv, 0.7 * nz, 0.05, 0.8, 0.3, 1.3, FV)
+    ref, refm, _ = _single(B, args, st, 10)
+    bounds = [S.slab_bounds(nz, 2, r) for r in range(2)]
+    sims = []
+    for d, (zb, nzl) in enumerate(bounds):
+        with torch.cuda.device(d):
+            sims.append(B.Cosenu(nzl, nv, *args[2:], use_torch_workspace=False, stream=torch.cuda.Stream(device=d), slab=(nz, zb)))
+    peers = [S._export(s) for s in sims]
+    for r, s in enumerate(sims):
+        S._link(s, peers[(r - 1) % 2], peers[(r + 1) % 2])
+    grp = S.ConcurrentSlabs.__new__(S.ConcurrentSlabs)
+    grp.nz_global, grp.nv, grp.bounds, grp.sims, grp._L = nz, nv, bounds, sims, sims[0]._L
+    grp.set_state(st)
+    grp.step(10)
+    grp.sync()
+    got = grp.get_state()
+    grp.close()
+    assert np.array_equal(got, ref)
