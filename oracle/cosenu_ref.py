@@ -30,7 +30,8 @@ _lib = None
 def lib():
     global _lib
     if _lib is None:
-        path = build_oracle.build()
+        # COSENU_REF_LIB: another build of the same source (the sanitizer build of tests/test_host_logic.py)
+        path = os.environ.get("COSENU_REF_LIB") or build_oracle.build()
         L = C.CDLL(path)
         dp = C.POINTER(C.c_double)
         L.cosenu_ref_create.restype = C.c_void_p

@@ -2,7 +2,6 @@
 
     python -m paper_2203_12866_b200.build [--force] [--verbose]
         -> paper_2203_12866_b200/libcosenu_b200.so     (the product: kernels + C ABI, include/cosenu.h)
-        -> paper_2203_12866_b200/libcosenu_probe.so    (host build of csrc/weno7_math.h for the CPU tests)
 
 nvcc cross-compiles without a GPU.  -lineinfo keeps the ncu source page mapped to csrc/.
 """
@@ -14,7 +13,6 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libcosenu_b200.so")
-PROBE = os.path.join(HERE, "libcosenu_probe.so")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
@@ -32,9 +30,6 @@ def build(force=False, verbose=False):
         cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
               ["-o", LIB, os.path.join(CSRC, "cosenu_api.cu")]
         subprocess.run(cmd, check=True)
-    if force or not _newer(PROBE, deps):
-        subprocess.run(["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-fPIC", "-shared", "-o", PROBE,
-                        os.path.join(CSRC, "host_probe.cpp")], check=True)
     return LIB
 
 

@@ -76,24 +76,50 @@ __device__ __forceinline__ double plen(double ee, double xx, double r, double i)
   return sqrt(fma(d, d, 4.0 * fma(r, r, i * i)));  // |P| of Eq. (4), un-normalised
 }
 
-// z-slab partial sums of |P|(z,v) and P0(z,v) per species: part[b][4][nv] (|P|_nu, P0_nu, |P|_nubar, P0_nubar)
-__global__ void diag_ref_kernel(const double* __restrict__ y, double* __restrict__ part, long long nz, int nv, int nvp,
-                                long long comp_stride, int g) {
+// z-slab partial sums of |P|(z,v) and P0(z,v) per species: part[b][4][nv] (|P|_nu, P0_nu, |P|_nubar, P0_nubar).
+// blockDim = DIAG_REF_ROWS x DIAG_REF_LANES: lane = beam (coalesced rows), DIAG_REF_ROWS rows of the block's z-range in flight
+// at once and two rows per thread and trip, so that the reads of a block cover the HBM latency; the row groups are summed
+// in a fixed order (reproducible).
+constexpr int DIAG_REF_ROWS = 4, DIAG_REF_LANES = 256;
+__global__ void __launch_bounds__(DIAG_REF_ROWS * DIAG_REF_LANES)
+    diag_ref_kernel(const double* __restrict__ y, double* __restrict__ part, long long nz, int nv, int nvp,
+                    long long comp_stride, int g) {
+  __shared__ double red[DIAG_REF_ROWS][4][DIAG_REF_LANES];
+  const int tj = threadIdx.x % DIAG_REF_LANES, tr = threadIdx.x / DIAG_REF_LANES;
   const long long rows_per = (nz + gridDim.x - 1) / gridDim.x;
   const long long z0 = blockIdx.x * rows_per, z1 = min(nz, z0 + rows_per);
-  for (int j = threadIdx.x; j < nv; j += blockDim.x) {
-    double a[4] = {0, 0, 0, 0};
-    for (long long iz = z0; iz < z1; ++iz) {
-      const double* q = y + (iz + g) * nvp + j;
+  for (int j0 = 0; j0 < nv; j0 += DIAG_REF_LANES) {
+    const int j = j0 + tj;
+    double a[4] = {0, 0, 0, 0}, b[4] = {0, 0, 0, 0};
+    if (j < nv) {
+      auto row = [&](long long iz, double (&acc)[4]) {
+        const double* q = y + (iz + g) * nvp + j;
+        double c[8];
 #pragma unroll
-      for (int s = 0; s < 2; ++s) {
-        const double ee = q[(4 * s) * comp_stride], xx = q[(4 * s + 1) * comp_stride];
-        a[2 * s] += plen(ee, xx, q[(4 * s + 2) * comp_stride], q[(4 * s + 3) * comp_stride]);
-        a[2 * s + 1] += ee + xx;
-      }
+        for (int k = 0; k < 8; ++k) c[k] = q[k * comp_stride];
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+          acc[2 * s] += plen(c[4 * s], c[4 * s + 1], c[4 * s + 2], c[4 * s + 3]);
+          acc[2 * s + 1] += c[4 * s] + c[4 * s + 1];
+        }
+      };
+      long long iz = z0 + tr;
+      for (; iz + DIAG_REF_ROWS < z1; iz += 2 * DIAG_REF_ROWS) { row(iz, a); row(iz + DIAG_REF_ROWS, b); }
+      if (iz < z1) row(iz, a);
     }
 #pragma unroll
-    for (int m = 0; m < 4; ++m) part[((long long)blockIdx.x * 4 + m) * nv + j] = a[m];
+    for (int m = 0; m < 4; ++m) red[tr][m][tj] = a[m] + b[m];
+    __syncthreads();
+    if (tr == 0 && j < nv) {
+#pragma unroll
+      for (int m = 0; m < 4; ++m) {
+        double sum = red[0][m][tj];
+#pragma unroll
+        for (int r = 1; r < DIAG_REF_ROWS; ++r) sum += red[r][m][tj];
+        part[((long long)blockIdx.x * 4 + m) * nv + j] = sum;
+      }
+    }
+    __syncthreads();
   }
 }
 

@@ -465,7 +465,7 @@ int one_step(cosenu* h) {
 // ---- diagnostics in four pieces, so that a decomposed run can put its reduction between them
 // (1) per-beam sums over my rows of |P_nu|, P0_nu, |P_nubar|, P0_nubar: out[4][nv]
 int ref_sums(cosenu* h, double* out) {
-  diag_ref_kernel<<<REF_BLOCKS, 256, 0, h->stream>>>(h->U, h->d_refpart, h->nz, h->nv, h->nvp, h->comp_stride, G);
+  diag_ref_kernel<<<REF_BLOCKS, DIAG_REF_ROWS * DIAG_REF_LANES, 0, h->stream>>>(h->U, h->d_refpart, h->nz, h->nv, h->nvp, h->comp_stride, G);
   CK(cudaGetLastError());
   h->launches++;
   std::vector<double> part((size_t)REF_BLOCKS * 4 * h->nv);

@@ -1,6 +1,7 @@
 // host_probe.cpp -- host-side build of the product's stencil arithmetic (weno7_math.h) so that the CPU
-// tests can check the formulas the kernels use against the oracle without a GPU.  Not used by the product.
-#include "weno7_math.h"
+// tests can check the formulas the kernels use against the oracle without a GPU.  Test code: built by tests/build_probe.py,
+// not by the product's build.
+#include "../paper_2203_12866_b200/csrc/weno7_math.h"
 
 extern "C" double cosenu_probe_weno7_face(const double* w7, double v, double eps) {
   // value of f = v u at the interface, as the kernels form it

@@ -103,11 +103,11 @@ def _advection_error_gpu(B, scheme, nz, eps_ko=None, weno_eps=None, T=2.0):
 def test_convergence_orders_gpu(B, golden):
     gv = golden("paper_values.txt")
     e = [_advection_error_gpu(B, FD, n, eps_ko=0.0) for n in (16, 32)]
-    assert abs(analysis.order_of_convergence(*e) - float(gv["order_fd4"])) < 0.25
+    assert abs(analysis.two_grid_order(*e) - float(gv["order_fd4"])) < 0.25
     e = [_advection_error_gpu(B, FV, n, weno_eps=1e30) for n in (16, 32)]
-    assert abs(analysis.order_of_convergence(*e) - float(gv["order_weno7"])) < 0.4
+    assert abs(analysis.two_grid_order(*e) - float(gv["order_weno7"])) < 0.4
     e = [_advection_error_gpu(B, FV, n, weno_eps=1e-6) for n in (16, 32)]
-    assert 5.0 < analysis.order_of_convergence(*e) < 8.5
+    assert 5.0 < analysis.two_grid_order(*e) < 8.5
 
 
 def test_conserved_quantity_scan_improves_with_resolution(B):
@@ -118,7 +118,60 @@ def test_conserved_quantity_scan_improves_with_resolution(B):
         seed=3, pert_amp=1e-3)
     assert rows[2]["dP_max"] < rows[1]["dP_max"] < rows[0]["dP_max"]
     assert all(r["dM0_max"] <= 1e-11 for r in rows)
-    assert analysis.kappa(rows[0]["dP_avg"], rows[1]["dP_avg"], rows[2]["dP_avg"]) > 1.0
+    assert analysis.richardson_ratio(rows[0]["dP_avg"], rows[1]["dP_avg"], rows[2]["dP_avg"]) > 1.0
+
+
+# the fiducial fast-conversion set-up of Section 5: Eq. (21) seed of 1e-2, alpha = 0.9; the domain length is
+# not printed: 1200, as in the other fiducial tests
+_FID_L, _FID_NV = 1200.0, 64
+
+
+def test_cfl_scan_fd_is_space_limited_fv_is_not(B):
+    """PAPER.md:280, Fig. 8(a,b): "doubling the resolution leads to considerable improvements in the errors for both FD and FV.
+    However, changing the value of C_CFL alone while keeping N_z unchanged ... does not affect the errors in the case of FD
+    whereas the same improves the numerical accuracy of FV"; panel (c): M0_3 stays at its initial value."""
+    cfls = [0.8, 0.4, 0.2]
+    res = {}
+    for scheme in (FD, FV):
+        mk = lambda nz, L, dt: B.Cosenu(nz, _FID_NV, L, dt, 0.0, 0.0, 1.0, scheme)
+        for nz in (1000, 2000):
+            res[scheme, nz] = analysis.cfl_scan(mk, nz, cfls, t_end=250.0, L=_FID_L)
+            assert all(abs(r["dM0_3"]) <= 1e-10 for r in res[scheme, nz])
+    for scheme in (FD, FV):
+        for a, b in zip(res[scheme, 1000], res[scheme, 2000]):                   # doubling N_z: considerable improvement
+            assert b["dP_max"] < 0.2 * a["dP_max"] and b["dP_avg"] < 0.3 * a["dP_avg"], (scheme, a, b)
+    for nz in (1000, 2000):                                                      # FD: C_CFL alone changes nothing (within 3 %)
+        e = [r["dP_max"] for r in res[FD, nz]]
+        assert max(e) / min(e) < 1.03, e
+        e = [r["dP_avg"] for r in res[FD, nz]]
+        assert max(e) / min(e) < 1.03, e
+    e = [r["dP_max"] for r in res[FV, 2000]]                                     # FV: a smaller C_CFL improves the accuracy
+    assert e[0] > 3.0 * e[1] and e[1] > e[2], e
+    e = [r["dP_max"] for r in res[FV, 1000]]
+    assert e[0] > 1.15 * e[1] and e[1] >= 0.99 * e[2], e
+
+
+def test_fixed_dt_scan_kappa(B):
+    """PAPER.md:280-294, Fig. 9: dt fixed such that N_z = 32768 has C_CFL = 1, 1000 iterations.  "For FD, the error decreases
+    monotonically as we increase N_z.  For FV, however, the error decreases until a saturation value (= 8962 here), after which
+    it stays constant"; kappa (Eq. 24) is about constant for FD, with a value like the order of accuracy of Section 4.1, while
+    for FV it "initially increases with the increase in N_z and then quickly approaches zero"."""
+    nzs = [512, 1024, 2048, 4096, 8192, 16384, 32768]
+    rows, kap = analysis.fixed_dt_scan(lambda nz, L, dt: B.Cosenu(nz, _FID_NV, L, dt, 0.0, 0.0, 1.0, FD), nzs, _FID_L)
+    assert rows[-1]["cfl"] == 1.0 and all(r["steps"] == 1000 for r in rows)
+    e = [r["dP_max"] for r in rows]
+    assert all(b < a for a, b in zip(e[:-1], e[1:])), e                          # monotonic
+    assert all(2.5 < k < 4.2 for k in kap), kap                                  # FD4 + third-order KO term: kappa ~ 3 - 3.7
+    # Eq. (C.3), three errors at one dt: the same spatial order
+    al = [analysis.order_of_convergence(e[i], e[i + 1], e[i + 2]) for i in range(len(e) - 2)]
+    assert all(2.5 < a < 4.2 for a in al), al
+    rows, kap = analysis.fixed_dt_scan(lambda nz, L, dt: B.Cosenu(nz, _FID_NV, L, dt, 0.0, 0.0, 1.0, FV), nzs, _FID_L)
+    e = [r["dP_max"] for r in rows]
+    assert kap[0] > 5.0 and kap[0] < kap[1] < kap[2] < 8.0, kap                  # rises towards the scheme's order 7
+    assert abs(kap[-1]) < 0.5 and abs(kap[-2]) < 0.5, kap                        # then -> 0: saturation
+    nsat = next(r["nz"] for r, k in zip(rows[1:], kap) if abs(k) < 0.5) // 2     # last N_z before the error stops falling
+    assert 4096 <= nsat <= 16384, nsat                                           # the paper's run: 8962
+    assert e[-1] < 1e-3 * e[2]
 
 
 @pytest.mark.parametrize("scheme", [FD, FV])

@@ -446,3 +446,30 @@ def test_capped_grid_is_bitwise_identical(B):
             outs.append((g.get_state(), g.get_moments()))
             g.close()
         assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+
+
+# ---- the hand-computed pins of tests/hand_pins.py, through the C ABI of the product
+def test_diagnostics_hand_values_gpu(B):
+    import hand_pins as H
+    g = B.Cosenu(H.NZ, H.NV, H.L, H.DT, 0.0, 0.0, 0.0, FD)
+    g.set_state(H.planted_state())
+    H.check_planted_diagnostics(g.diagnostics())
+    g.close()
+
+
+@pytest.mark.parametrize("scheme", [FD, FV])
+def test_eq21_seed_profile_hand_values_gpu(B, scheme):
+    import hand_pins as H
+    nz, L = H.E21_GRID[scheme]
+    g = B.Cosenu(nz, 6, L, 0.5, 0.0, 0.0, 1.0, scheme)
+    g.init(1, pert_amp=H.E21_AMP, pert_kind=2)
+    H.check_eq21_state(g.get_state(), scheme)
+    g.close()
+
+
+def test_band_limited_seed_has_16_equal_modes_gpu(B):
+    import hand_pins as H
+    g = B.Cosenu(256, 4, 256.0, 0.4, 0.0, 0.0, 1.0, FV)
+    g.init(11, pert_amp=1e-3, pert_kind=1)
+    H.check_band_limited(g.get_state(), 1e-3)
+    g.close()

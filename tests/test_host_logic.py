@@ -15,8 +15,9 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 @pytest.fixture(scope="module")
 def libs():
+    import build_probe
     pbuild.build()
-    return C.CDLL(pbuild.LIB), C.CDLL(pbuild.PROBE)
+    return C.CDLL(pbuild.LIB), C.CDLL(build_probe.build())
 
 
 def test_library_exports_every_declared_symbol(libs):
@@ -171,11 +172,55 @@ def test_analysis_dP_map_matches_the_diagnostics_definition():
 
 
 def test_analysis_estimators_on_known_sequences():
-    """E2 (Eq. 15), the order estimator (Eq. C.3) and kappa (Eq. 24) on sequences whose answers are known."""
+    """E2 (Eq. 15), kappa (Eq. 24) and the three-error order estimator (Eq. C.3) as printed, on
+    sequences whose answers are known; plus the two textbook estimators that keep their own names."""
     from paper_2203_12866_b200 import analysis
     assert abs(analysis.e2_norm([1.0, 2.0, 3.0], [1.0, 2.0, 5.0]) - np.sqrt(4.0 / 3.0)) < 1e-15
+    # Eq. (24): dP_max halves four times when N_z doubles -> kappa = 4; equal errors (time-integration floor) -> kappa = 0
+    assert analysis.kappa(3.2e-3, 2.0e-4) == pytest.approx(4.0, abs=1e-12)
+    assert analysis.kappa(2.5e-13, 2.5e-13) == 0.0
+    assert analysis.kappa(1.0, 8.0) == pytest.approx(-3.0, abs=1e-12)
     for p in (3.0, 4.0, 7.0):
-        assert abs(analysis.order_of_convergence(5.0, 5.0 / 2 ** p) - p) < 1e-12          # errors ~ h^p, h halved
+        # Eq. (C.2): E_i = C_z (dz_0 / r^i)^alpha + C_t dt^beta with one dt for all i: the constant cancels in Eq. (C.3)
+        for r in (2.0, 3.0):
+            E = [0.7 * (0.4 / r ** i) ** p + 0.123 for i in range(3)]
+            assert abs(analysis.order_of_convergence(*E, ratio=r) - p) < 1e-9
+        # whereas the two-error ratio is fooled by that constant, and exact without it
+        assert abs(analysis.two_grid_order(5.0, 5.0 / 2 ** p) - p) < 1e-12
+        assert analysis.two_grid_order(5.0 + 0.123, 5.0 / 2 ** p + 0.123) < p - 0.05
         q = [1.0 + 0.3 * h ** p for h in (0.4, 0.2, 0.1)]                                   # q(h) = q* + C h^p
-        assert abs(analysis.kappa(*q) - 2 ** p) < 1e-6 * 2 ** p                             # kappa -> 2^p
-    assert analysis.kappa(1.0, 2.0, 2.0) == float("inf")
+        assert abs(analysis.richardson_ratio(*q) - 2 ** p) < 1e-6 * 2 ** p
+    assert analysis.richardson_ratio(1.0, 2.0, 2.0) == float("inf")
+
+
+def test_oracle_under_address_and_undefined_behaviour_sanitizers(tmp_path):
+    """SURVEY.md section 5 (race detection / sanitizers): the oracle built with -fsanitize=address,undefined runs the FD closed
+    form (P3), the WENO linear limit (P6) and the brute-force commutator / moments (P9) pins without a report.  The sanitized
+    library is loaded in a child process (ASan must be the first DSO), which runs those pins of tests/test_oracle_pins.py."""
+    import shutil
+    import subprocess
+    import sys
+    if shutil.which("g++") is None:
+        pytest.skip("no g++")
+    out = tmp_path / "libcosenu_ref_asan.so"
+    src = os.path.join(ROOT, "oracle", "cosenu_ref.cpp")
+    r = subprocess.run(["g++", "-std=c++17", "-O1", "-g", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
+                        "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer",
+                        "-o", str(out), src], capture_output=True, text=True)
+    if r.returncode != 0 and "sanitize" in (r.stderr or ""):
+        pytest.skip("this g++ has no sanitizer runtime: " + r.stderr[-200:])
+    assert r.returncode == 0, r.stderr
+    asan = subprocess.run(["g++", "-print-file-name=libasan.so"], capture_output=True, text=True).stdout.strip()
+    if not os.path.isabs(asan):
+        pytest.skip("libasan.so not found")
+    env = dict(os.environ, LD_PRELOAD=asan, COSENU_REF_LIB=str(out),
+               ASAN_OPTIONS="detect_leaks=0:halt_on_error=1:abort_on_error=0", UBSAN_OPTIONS="halt_on_error=1:print_stacktrace=1",
+               OMP_NUM_THREADS="2")
+    r = subprocess.run([sys.executable, "-m", "pytest", "-x", "-q", "-p", "no:cacheprovider",
+                        os.path.join(ROOT, "tests", "test_oracle_pins.py"),
+                        "-k", "P3_fd_ko_discrete_closed_form or P6_weno_linear_limit or P9_commutator or diagnostics_hand_values"],
+                       capture_output=True, text=True, env=env, cwd=ROOT, timeout=600)
+    tail = (r.stdout or "")[-1500:] + (r.stderr or "")[-1500:]
+    assert r.returncode == 0, tail
+    assert "ERROR: AddressSanitizer" not in tail and "runtime error" not in tail, tail
+    assert "passed" in r.stdout

@@ -700,3 +700,34 @@ def test_boxcar_advection_error_is_half_and_resolution_independent(scheme):
     Gibbs oscillations, FV does not.  (Domain length not printed: 1200, i.e. dz = 0.6 at the paper's N_z = 2000.)"""
     mk = lambda nz, nv, L, dt, s: R.RefSim(nz, nv, L, dt, 0.0, 0.0, 0.0, s)
     check_boxcar([boxcar_run(mk, scheme, nz, T=90.0) for nz in (500, 1000)], scheme)
+
+
+# ----------------------------------------------------------------------------- hand-computed pins of the diagnostics and seeds
+def test_diagnostics_hand_values_eq22_eq23():
+    """dP_avg (Eq. 23), dP_max (Eq. 22), trace_dev_max, ex_abs_max on a planted two-beam state with unequal weights g_v: the
+    expectations are literals derived by hand in tests/hand_pins.py (a wrong weighting or normalisation fails them)."""
+    import hand_pins as H
+    sim = R.RefSim(H.NZ, H.NV, H.L, H.DT, 0.0, 0.0, 0.0, FD)
+    sim.set_state(H.planted_state())
+    H.check_planted_diagnostics(sim.diagnostics())
+    sim.close()
+
+
+@pytest.mark.parametrize("scheme", [FD, FV])
+def test_eq21_seed_profile_hand_values(scheme):
+    """Eq. (21): eps(z) = amp exp(-(z - L/2)^2/50) at offsets 0, +-5, +-10 equals amp {1, e^-1/2, e^-2} on
+    the FD grid (z_i = i dz) and on the FV grid (cell centres); rho_ex = g eps/2, rho_ee - rho_xx = g sqrt(1 - eps^2)."""
+    import hand_pins as H
+    nz, L = H.E21_GRID[scheme]
+    sim = R.RefSim(nz, 6, L, 0.5, 0.0, 0.0, 1.0, scheme)
+    sim.init(1, pert_amp=H.E21_AMP, pert_kind=2)
+    H.check_eq21_state(sim.get_state(), scheme)
+    sim.close()
+
+
+def test_band_limited_seed_has_16_equal_modes():
+    import hand_pins as H
+    sim = R.RefSim(256, 4, 256.0, 0.4, 0.0, 0.0, 1.0, FV)
+    sim.init(11, pert_amp=1e-3, pert_kind=1)
+    H.check_band_limited(sim.get_state(), 1e-3)
+    sim.close()
