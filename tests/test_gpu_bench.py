@@ -70,3 +70,15 @@ def test_bench_secondary_lines():
     assert s3["config"]["scheme"] == "FD4_KO3" and s3["value"] > 1e9
     for x in d["secondary"][1:]:
         assert 0 < x["graph_replay"]["ms_per_step"] <= 1.5 * x["launch_by_launch"]["ms_per_step"]
+
+
+def test_slab_bitwise_check_of_the_multi_gpu_line():
+    """bench.py's N > 1 line carries `slab_check` (a reduced free-running slab run against the single domain, bit for bit);
+    with one rank the slab is linked to itself."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    sys.path.insert(0, ROOT)
+    import bench
+    r = bench.slab_bitwise_check(1, 0)
+    assert r["bitwise_equal_to_single_domain"] is True and r["halo_wait_failed"] is False and r["slabs"] == 1
