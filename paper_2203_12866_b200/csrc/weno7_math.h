@@ -71,7 +71,17 @@ COSENU_HD Weno7Beam weno7_beam(double v, double eps) {
   // eps / v^2, kept below 1e45 so that the products of six q_r stay in range for every accepted eps (1e-40 .. 1e30), also
   // on a beam with v = 0 exactly (vertex-centred grids); there the flux is multiplied by |v| = 0 afterwards
   const double v2 = v * v;
-  double ev = eps / (v2 < 1e-300 ? 1e-300 : v2);
+  const double v2c = v2 < 1e-300 ? 1e-300 : v2;
+#ifdef __CUDA_ARCH__
+  // eps / v^2 once per beam and work item: the hardware seed + one third-order step (as in fast_half_rcp; ~1 ulp) instead of
+  // the ~40 dependent instructions of an IEEE division, which the marching warps would run serially at every item
+  double x;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(v2c));
+  const double e = fma(-v2c, x, 1.0);
+  double ev = eps * fma(x, fma(e, e, e), x);
+#else
+  double ev = eps / v2c;
+#endif
   if (ev > 1e45) ev = 1e45;
   Weno7Beam b;
   b.e0 = ev * 2.9580398915498080213;   // sqrt(35/4)

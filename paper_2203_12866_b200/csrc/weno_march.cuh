@@ -96,12 +96,25 @@ __device__ __forceinline__ void weno_march(uint32_t Ty0, uint32_t Tk0, bool neg,
   double Flo = 0.0, Fhi = 0.0;
   // X[idx] (X = c, D, E, T) is needed by the upward march at step idx - (6, 5, 4, 3) and by the downward one at step
   // NI - 1 - idx; whichever comes first (the upward march goes first within a step) forms it, once.
+  // The shared-memory loads are issued PD steps ahead of their use: a load cannot pass an earlier store to shared memory (the
+  // flux differences of the previous interfaces), so a load issued where its cell is first needed would wait for the end of the
+  // previous interface's dependency chain and serialise the two marches.
+  constexpr int PD = 2;
+  auto up_loads = [&](int s) {     // the cell the upward march needs at step s, if it is the upward march's to load
+    if (s < NLO && 2 * s + 6 <= NI - 1) c[s + 6] = cell(s + 6);
+  };
+  auto down_loads = [&](int s) {   // likewise for the downward march (interface m = NI - 1 - s, new cell m)
+    if (s < NI - NLO && (NI - 1 - s) - 6 > s) c[NI - 1 - s] = cell(NI - 1 - s);
+  };
+#pragma unroll
+  for (int s = 0; s < PD; ++s) { up_loads(s); down_loads(s); }
 #pragma unroll
   for (int s = 0; s < NLO; ++s) {
     if (s == 1) mbar_wait(bar_free, par_free);
+    up_loads(s + PD);
+    down_loads(s + PD);
     {   // upward march, interface m = s: the new cell is m + 6
       const int m = s;
-      if (2 * s + 6 <= NI - 1) c[m + 6] = cell(m + 6);
       if (2 * s + 5 <= NI - 1) D[m + 5] = c[m + 6] - c[m + 5];
       if (2 * s + 4 <= NI - 1) E[m + 4] = D[m + 5] - D[m + 4];
       if (2 * s + 3 <= NI - 1) { T[m + 3] = E[m + 4] - E[m + 3]; TT[m + 3] = T[m + 3] * T[m + 3]; }
@@ -112,7 +125,6 @@ __device__ __forceinline__ void weno_march(uint32_t Ty0, uint32_t Tk0, bool neg,
     }
     if (s < NI - NLO) {   // downward march, interface m = NI - 1 - s: the new cell is m
       const int m = NI - 1 - s;
-      if (m - 6 > s) c[m] = cell(m);
       if (m - 5 > s) D[m] = c[m + 1] - c[m];
       if (m - 4 > s) E[m] = D[m + 1] - D[m];
       if (m - 3 > s) { T[m] = E[m + 1] - E[m]; TT[m] = T[m] * T[m]; }
