@@ -91,6 +91,27 @@ COSENU_HD Weno7Beam weno7_beam(double v, double eps) {
   return b;
 }
 
+// the 19 constants of weno7_core.  On the device they live in the constant bank, so that every DFMA takes its constant as an
+// operand (c[bank][offset]); as 64-bit immediates they would be re-materialised into uniform registers (two UMOV each) at
+// every work item.  k_r = 1/sqrt(d_r) = sqrt(35/4), sqrt(35/18), sqrt(35/12), sqrt(35).
+enum { C_1_3, C_M5_6, C_M1_6, C_2_3, C_7_6, C_11_6, C_1_6, C_240K0, C_260K0, C_781K0, C_240K1, C_260K1, C_781K1,
+       C_240K2, C_260K2, C_781K2, C_240K3, C_260K3, C_781K3, C_COUNT };
+#define COSENU_WENO_CONSTANTS                                                                                              \
+  {1.0 / 3.0, -5.0 / 6.0, -1.0 / 6.0, 2.0 / 3.0, 7.0 / 6.0, 11.0 / 6.0, 1.0 / 6.0,                                          \
+   240.0 * 2.9580398915498080213, 260.0 * 2.9580398915498080213, (781.0 / 3.0) * 2.9580398915498080213,                   \
+   240.0 * 1.3944333775567926, 260.0 * 1.3944333775567926, (781.0 / 3.0) * 1.3944333775567926,                            \
+   240.0 * 1.7078251276599330, 260.0 * 1.7078251276599330, (781.0 / 3.0) * 1.7078251276599330,                            \
+   240.0 * 5.9160797830996160426, 260.0 * 5.9160797830996160426, (781.0 / 3.0) * 5.9160797830996160426}
+#ifdef __CUDACC__
+__constant__ double weno_const_dev[C_COUNT] = COSENU_WENO_CONSTANTS;
+#endif
+static constexpr double weno_const_host[C_COUNT] = COSENU_WENO_CONSTANTS;
+#ifdef __CUDA_ARCH__
+#define WC(i) weno_const_dev[i]
+#else
+#define WC(i) weno_const_host[i]
+#endif
+
 // the part of Algorithm 1 after the undivided differences: D[0..5], E[0..4], T[0..3] of the 7 cells
 // w[0..6] (D_k = w[k+1]-w[k], E_k = D[k+1]-D[k], T_k = E[k+1]-E[k]); ui = w[3]; TTk = T_k^2 (shared
 // between neighbouring interfaces by weno7_face2).
@@ -98,25 +119,23 @@ COSENU_HD double weno7_core(double ui, double D0, double D1, double D2, double D
                             double E3, double E4, double T0, double T3, double TT0, double TT1, double TT2, double TT3,
                             const Weno7Beam& bm) {
   // A_r, s_r per sub-stencil: (x, p, q, t) = (D[3-r], E[3-r], E[4-r], T[3-r])
-  const double A0 = fma(1.0 / 3.0, E4, fma(-5.0 / 6.0, E3, D3));
-  const double A1 = fma(-1.0 / 6.0, E3, fma(2.0 / 3.0, E2, D2));
-  const double A2 = fma(1.0 / 3.0, E2, fma(7.0 / 6.0, E1, D1));
-  const double A3 = fma(11.0 / 6.0, E1, fma(2.0 / 3.0, E0, D0));
+  const double A0 = fma(WC(C_1_3), E4, fma(WC(C_M5_6), E3, D3));
+  const double A1 = fma(WC(C_M1_6), E3, fma(WC(C_2_3), E2, D2));
+  const double A2 = fma(WC(C_1_3), E2, fma(WC(C_7_6), E1, D1));
+  const double A3 = fma(WC(C_11_6), E1, fma(WC(C_2_3), E0, D0));
   const double s0 = E3 - T3, s3 = E1 + T0;   // s1 = s2 = E2
   const double ss12 = E2 * E2;
   // qs_r = (240 A^2 + 260 s^2 + (781/3) t^2 + eps/v^2) / sqrt(d_r)
-  constexpr double k0 = 2.9580398915498080213, k1 = 1.3944333775567926, k2 = 1.7078251276599330,
-                   k3 = 5.9160797830996160426;
-  const double q0 = fma(240.0 * k0, A0 * A0, fma(260.0 * k0, s0 * s0, fma((781.0 / 3.0) * k0, TT3, bm.e0)));
-  const double q1 = fma(240.0 * k1, A1 * A1, fma(260.0 * k1, ss12, fma((781.0 / 3.0) * k1, TT2, bm.e1)));
-  const double q2 = fma(240.0 * k2, A2 * A2, fma(260.0 * k2, ss12, fma((781.0 / 3.0) * k2, TT1, bm.e2)));
-  const double q3 = fma(240.0 * k3, A3 * A3, fma(260.0 * k3, s3 * s3, fma((781.0 / 3.0) * k3, TT0, bm.e3)));
+  const double q0 = fma(WC(C_240K0), A0 * A0, fma(WC(C_260K0), s0 * s0, fma(WC(C_781K0), TT3, bm.e0)));
+  const double q1 = fma(WC(C_240K1), A1 * A1, fma(WC(C_260K1), ss12, fma(WC(C_781K1), TT2, bm.e1)));
+  const double q2 = fma(WC(C_240K2), A2 * A2, fma(WC(C_260K2), ss12, fma(WC(C_781K2), TT1, bm.e2)));
+  const double q3 = fma(WC(C_240K3), A3 * A3, fma(WC(C_260K3), s3 * s3, fma(WC(C_781K3), TT0, bm.e3)));
   const double Q0 = q0 * q0, Q1 = q1 * q1, Q2 = q2 * q2, Q3 = q3 * q3;
   const double Q01 = Q0 * Q1, Q23 = Q2 * Q3;
   // P_0 = Q1 Q23, P_1 = Q0 Q23, P_2 = Q01 Q3, P_3 = Q01 Q2, grouped:
   //   den = Q23 (Q0 + Q1) + Q01 (Q2 + Q3),  num = Q23 (Q1 c0 + Q0 c1) + Q01 (Q3 c2 + Q2 c3)
-  const double c0 = fma(1.0 / 6.0, s0, A0), c1 = fma(1.0 / 6.0, E2, A1), c2 = fma(1.0 / 6.0, E2, A2),
-               c3 = fma(1.0 / 6.0, s3, A3);
+  const double c0 = fma(WC(C_1_6), s0, A0), c1 = fma(WC(C_1_6), E2, A1), c2 = fma(WC(C_1_6), E2, A2),
+               c3 = fma(WC(C_1_6), s3, A3);
   const double den = fma(Q01, Q2 + Q3, Q23 * (Q0 + Q1));
   const double num = fma(Q01, fma(Q3, c2, Q2 * c3), Q23 * fma(Q1, c0, Q0 * c1));
   return fma(num, fast_half_rcp(den), ui);

@@ -33,8 +33,8 @@ constexpr int MNW = 8, MNC = 4;         // WENO warps (one per component), combi
 constexpr int MRC = MTZ / MNC;          // rows per combine warp
 constexpr int MARCH_THREADS = (MNW + MNC + 4) * 32;   // + the DMA warp and three idle warps (a full warpgroup for setmaxnreg)
 // registers per thread after the roles have split (the kernel is launched with 512 threads x 128 registers; every SM
-// sub-partition holds two WENO warps, one combine warp and one warp of the DMA group): 2 x 168 + 128 + 40 <= 512
-constexpr int MREG_WENO = 168, MREG_DMA = 40;
+// sub-partition holds two WENO warps, one combine warp and one warp of the DMA group): 2 x 160 + 152 + 40 = 512
+constexpr int MREG_WENO = 160, MREG_COMB = 152, MREG_DMA = 40;
 
 struct MarchSmem {
   static constexpr uint32_t YTILE = 8u * MROWS * VC * 8u;
@@ -246,6 +246,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, 1)
   }
 
   // =========================================================================== combine warps: rows 4q .. 4q+3
+  asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(MREG_COMB));
   const int q = warp - MNW;
   const int row0 = q * MRC;
   double msum[6 * MRC];
@@ -280,33 +281,27 @@ __global__ void __launch_bounds__(MARCH_THREADS, 1)
     const double cf = fabs(v) * p.ninv_dz;   // -|v|/dz: the flux differences are taken along the march (upwind to downwind)
     auto mom = [&](int s, int qq) { return __shfl_sync(0xffffffffu, min_cur, s * 6 + qq); };
 
+    // the cell values of my rows are read as soon as the stage-input tile is there -- while the WENO warps still march through
+    // it -- and the slot is released at once: it is then free the moment the marches end, and the TMA load of the item after
+    // next has a whole item time (one SM's share of HBM needs 1.1 us for a tile, an item takes 2.5-3 us)
+    mbar_wait(b_full_y + 8 * sy, par);
+    double yca[MRC][8];
+#pragma unroll
+    for (int s = 0; s < MRC; ++s)
+#pragma unroll
+      for (int c = 0; c < 8; ++c) yca[s][c] = lds(Ty + ((c * ROWS + row0 + s + H) * VC) * 8);
+    __syncwarp();
+    if (lane == 0) mbar_arrive(b_empty_y + 8 * sy);
     mbar_wait(b_k_ready + 8 * su, par);
-    mbar_wait(b_full_y + 8 * sy, par);    // already complete (the WENO warps have consumed the slot): orders my reads after the TMA writes
     mbar_wait(b_full_a + 8 * su, par);
-    double ycl[8];
 #pragma unroll
     for (int s = 0; s < MRC; ++s) {
       const int row = row0 + s;
       const long long iz = iz0 + row;
       const bool act = active && (iz < p.nz);
-      const int tr = row + H;
       double yc[8], k[8];
-      if (s < MRC - 2) {
 #pragma unroll
-        for (int c = 0; c < 8; ++c) yc[c] = lds(Ty + ((c * ROWS + tr) * VC) * 8);
-      } else if (s == MRC - 2) {
-        // the cell values of the last two rows are read together, so that the stage-input slot is released half way
-        // through the combine step (the TMA load of the item after next waits for it)
-#pragma unroll
-        for (int c = 0; c < 8; ++c) yc[c] = lds(Ty + ((c * ROWS + tr) * VC) * 8);
-#pragma unroll
-        for (int c = 0; c < 8; ++c) ycl[c] = lds(Ty + ((c * ROWS + tr + 1) * VC) * 8);
-        __syncwarp();
-        if (lane == 0) mbar_arrive(b_empty_y + 8 * sy);
-      } else {
-#pragma unroll
-        for (int c = 0; c < 8; ++c) yc[c] = ycl[c];
-      }
+      for (int c = 0; c < 8; ++c) yc[c] = yca[s][c];
       // ---- S3: Hamiltonian from the moments (mu folded in), commutator
       {
         const double Sd = fma(-v, mom(s, 1), mom(s, 0));
@@ -339,7 +334,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, 1)
         const double o = fma(p.cy, k[c], base);
         sts(Tu + cell, o);
         if constexpr (KIND == MID_P) sts(Tk + cell, (fma(2.0, o, yc[c]) - u0v) * (1.0 / 3.0));   // P; yc = Y2, o = Y3
-        out[c] = act ? o : 0.0;
+        out[c] = o;
       }
       if (act && (iz < G || iz >= p.nz - G)) {
         if (iz < G) {
@@ -356,6 +351,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, 1)
       // ---- S5: velocity moments of the produced state, D = rho - rhobar^*
       {
         double dd = (out[0] - out[1]) - (out[4] - out[5]), dr = out[2] - out[6], di = out[3] + out[7];
+        if (!act) { dd = 0.0; dr = 0.0; di = 0.0; }   // padding lanes / rows past the grid hold zero-filled cells: no contribution
         if (p.quad != 0) { dd *= wq; dr *= wq; di *= wq; }
         msum[6 * s + 0] += dd;
         msum[6 * s + 1] = fma(v, dd, msum[6 * s + 1]);
