@@ -236,6 +236,55 @@ int cosenu_slab_stage(cosenu_t* h, int32_t k);
 /* 1 if a halo wait of this handle ever timed out (a neighbour did not arrive within ~4 s); synchronises. */
 int cosenu_slab_wait_failed(cosenu_t* h, int32_t* failed);
 
+/* ===================================================================================================
+ * One call that allocates nothing on the device.
+ *
+ * Who it is for.  Everything above needs a workspace, and somebody has to cudaMalloc it.  Some code that wants a
+ * diagnostic of a state cannot do that where it runs:
+ *   - a monitor hooked into a production time loop whose process has handed the GPU's memory to a pooling allocator
+ *     (PyTorch's caching allocator, RMM, an application arena).  At the 262144 x 512 configuration the solver's own
+ *     workspace is 34 GB; a raw cudaMalloc beside the pool either fails for lack of free memory or takes memory the
+ *     pool's bookkeeping knows nothing about;
+ *   - a monitor that runs while z-slab handles free-run on other streams of the same GPU.  cudaFree (and, depending
+ *     on the driver, cudaMalloc) waits for the whole device.  A host thread stuck in that wait cannot enqueue the next
+ *     stage of its own slab, the neighbouring slab's kernel spins on the ghost rows that stage would deliver, gives up
+ *     after about 4 s, and the run is flagged invalid (cosenu_slab_wait_failed).
+ * For them: the per-beam z-sums of the polarisation-vector length and of the trace, the quantities cosenu_slab_ref_sums
+ * returns and from which the references |P|_0(v), P0_0(v) of Eq. (22), (23) (Eq. 4)
+ * are formed, computed from a state that already sits in device memory.
+ *
+ *   dev_state  DEVICE pointer, caller-owned, read only: a state in the canonical layout double[8][nz][nv] (dense).
+ *   dev_out    DEVICE pointer, caller-owned: double[4][nv], overwritten with
+ *              out[0][j] = sum_z |P_nu|(z, v_j),    out[1][j] = sum_z (rho_ee + rho_xx)(z, v_j),
+ *              out[2][j], out[3][j] = the same for rhobar;   |P| = sqrt((ee - xx)^2 + 4 (Re ex^2 + Im ex^2)).
+ *   cuda_stream  a cudaStream_t (NULL = the legacy default stream).  The two kernel launches are enqueued on it and
+ *              the call returns without waiting; dev_out is valid once the stream has reached that point.
+ *   Both buffers must belong to the device that is CURRENT when the call is made (managed memory is accepted too).
+ *
+ * Where the scratch memory comes from.  The per-block partial sums go into a fixed array compiled into the library
+ * (148 x 4 x COSENU_STATIC_MAX_NV doubles = 2.3 MiB).  Every GPU on which a process loads this library's device code
+ * holds one copy until the process exits, whether or not this call is ever made.
+ * Limits: 1 <= nv <= COSENU_STATIC_MAX_NV and 1 <= nz <= 2^40; anything else returns COSENU_EINVAL (the text names
+ * the limit) and launches nothing.  Wider v-grids have to use a handle (cosenu_slab_ref_sums).
+ * No allocation: the call makes no cudaMalloc, cudaFree, cudaMallocAsync or other allocating CUDA / library call, on
+ * the first call or later.  The FIRST call on each device additionally looks up where that device's copy of the array
+ * lives (cudaGetSymbolAddress, with that device current, serialised by a mutex) and remembers it; make that first call
+ * before any stream capture begins in the process.
+ * Sharing: all calls on a device use the SAME array, and it keeps whatever the last call left in it.  Nothing in it
+ * has to start at zero (the first launch overwrites every entry the second one reads, for the nv of that call), so
+ * successive calls with different nz / nv on one stream are fine.  Two calls that can overlap on the GPU (different
+ * streams without an event between them, or two host threads on different streams) race on the array and both results
+ * are garbage: order them yourself.  Separate processes have separate copies.
+ * Accuracy: not bit-identical to cosenu_slab_ref_sums (which sums the same 148 partials on the host in long double);
+ * the two agree to a few ulp of each sum.
+ * Errors: returns a COSENU_* code; the text of the calling thread's last failure is at
+ * cosenu_beam_sums_static_error() (valid until that thread's next call; empty if none failed).  Host pointers, a
+ * buffer of another device, nv or nz out of range -> COSENU_EINVAL; CUDA failures (including: no device) -> COSENU_ECUDA.
+ * =================================================================================================== */
+#define COSENU_STATIC_MAX_NV 512
+int cosenu_beam_sums_static(const double* dev_state, int64_t nz, int32_t nv, double* dev_out, void* cuda_stream);
+const char* cosenu_beam_sums_static_error(void);
+
 #ifdef __cplusplus
 }
 #endif

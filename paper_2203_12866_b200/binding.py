@@ -23,7 +23,9 @@ SYMBOLS = ["cosenu_create", "cosenu_workspace_bytes", "cosenu_attach", "cosenu_s
            "cosenu_sync", "cosenu_launch_count", "cosenu_stage_times", "cosenu_destroy", "cosenu_last_error",
            "cosenu_create_slab", "cosenu_slab_export", "cosenu_slab_link", "cosenu_slab_push_ghosts",
            "cosenu_slab_ref_sums", "cosenu_slab_set_ref_sums", "cosenu_slab_diag_sums", "cosenu_slab_diag_finish",
-           "cosenu_slab_step_group", "cosenu_slab_stage", "cosenu_slab_wait_failed"]
+           "cosenu_slab_step_group", "cosenu_slab_stage", "cosenu_slab_wait_failed",
+           "cosenu_beam_sums_static", "cosenu_beam_sums_static_error"]
+STATIC_MAX_NV = 512   # COSENU_STATIC_MAX_NV of include/cosenu.h
 
 
 class Diag(C.Structure):
@@ -92,6 +94,9 @@ def load():
     L.cosenu_slab_step_group.argtypes = [C.POINTER(C.c_void_p), C.c_int32, C.c_int64]
     L.cosenu_slab_stage.argtypes = [C.c_void_p, C.c_int32]
     L.cosenu_slab_wait_failed.argtypes = [C.c_void_p, C.POINTER(C.c_int32)]
+    L.cosenu_beam_sums_static.argtypes = [C.c_void_p, C.c_int64, C.c_int32, C.c_void_p, C.c_void_p]
+    L.cosenu_beam_sums_static_error.restype = C.c_char_p
+    L.cosenu_beam_sums_static_error.argtypes = []
     _lib = L
     return L
 
@@ -100,6 +105,34 @@ class CosenuError(RuntimeError):
     def __init__(self, code, msg):
         super().__init__("cosenu error %d: %s" % (code, msg))
         self.code = code
+
+
+def beam_sums_static(dev_state, dev_out, stream=None):
+    """cosenu_beam_sums_static: per-beam z-sums of |P_nu|, P0_nu, |P_nubar|, P0_nubar of a state that is already on the GPU,
+    without any device allocation inside the library (its scratch is an array built into the .so).
+
+    For callers that cannot cudaMalloc where they run: a monitor inside a process whose pooling allocator owns the
+    GPU's memory, or one running beside free-running slab handles, where the device-wide wait of cudaFree / cudaMalloc
+    would stall a neighbour's halo wait into its time-out.  Both tensors are the caller's: `dev_state` a contiguous CUDA
+    float64 tensor (8, nz, nv) with nv <= STATIC_MAX_NV, `dev_out` a contiguous CUDA float64 tensor (4, nv) that is
+    overwritten.  This wrapper allocates nothing either; it only passes pointers.  The launches go to `stream` (default:
+    torch's current stream) and the call does not wait for them.  All calls on a device share one scratch array: calls
+    that may overlap on the GPU must be ordered by the caller.  The first call on a device also looks the array's address
+    up; make it outside any stream capture."""
+    import torch
+    L = load()
+    for t in (dev_state, dev_out):
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+            raise TypeError("beam_sums_static takes contiguous CUDA float64 tensors")
+    if dev_state.dim() != 3 or dev_state.shape[0] != 8 or tuple(dev_out.shape) != (4, dev_state.shape[2]):
+        raise ValueError("beam_sums_static: dev_state must be (8, nz, nv) and dev_out (4, nv)")
+    st = stream if stream is not None else torch.cuda.current_stream(dev_state.device)
+    with torch.cuda.device(dev_state.device):   # the buffers' device must be the current one
+        rc = L.cosenu_beam_sums_static(dev_state.data_ptr(), dev_state.shape[1], dev_state.shape[2], dev_out.data_ptr(),
+                                       st.cuda_stream)
+    if rc != 0:
+        raise CosenuError(rc, L.cosenu_beam_sums_static_error().decode())
+    return dev_out
 
 
 class Cosenu:

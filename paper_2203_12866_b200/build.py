@@ -14,6 +14,10 @@ CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libcosenu_b200.so")
 
+# translation units of the library: the handle-based API with all stage kernels, and the allocation-free
+# cosenu_beam_sums_static, which keeps its file-scope scratch array and the host code that looks its address up in one file
+UNITS = ["cosenu_api.cu", "beam_sums_static.cu"]
+
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
 
@@ -28,7 +32,7 @@ def build(force=False, verbose=False):
     if force or not _newer(LIB, deps):
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
-              ["-o", LIB, os.path.join(CSRC, "cosenu_api.cu")]
+              ["-o", LIB] + [os.path.join(CSRC, f) for f in UNITS]
         subprocess.run(cmd, check=True)
     return LIB
 
