@@ -127,10 +127,14 @@ struct DeviceGuard {
 
 // z-slab: a halo wait that gave up (a neighbour that never delivered its rows) leaves stale ghost rows behind: every call
 // that hands results to the caller reports it.  The stream is idle here (the callers have just synchronised it).
+// The flag is read on the handle's OWN stream: a plain cudaMemcpy runs on the legacy default stream and would first wait
+// for every blocking stream of the device -- i.e. for another slab's queued stages, which in turn spin on the stage this
+// thread has not launched yet, until their halo wait times out.
 int halo_check(cosenu* h, const char* who) {
   if (!h->slab || !h->maps_ready) return COSENU_OK;
   int v = 0;
-  CK(cudaMemcpy(&v, h->d_err, sizeof(int), cudaMemcpyDeviceToHost));
+  CK(cudaMemcpyAsync(&v, h->d_err, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
   if (v) return fail(h, COSENU_ESTATE, std::string(who) + ": a halo wait timed out (a neighbouring slab never delivered its ghost rows); the state is invalid");
   return COSENU_OK;
 }

@@ -287,11 +287,14 @@ class ConcurrentSlabs(SlabGroup):
     protocol of a multi-GPU run (RAW wait, WAR argument of DESIGN.md section 8) on one GPU.
     """
 
-    def __init__(self, nslabs, nz_global, nv, L, dt, omega, theta, mu, scheme, max_ctas, bounds=None, **opts):
+    def __init__(self, nslabs, nz_global, nv, L, dt, omega, theta, mu, scheme, max_ctas, bounds=None,
+                 blocking_streams=False, **opts):
+        """blocking_streams: every handle creates its own plain cudaStreamCreate stream (one that synchronises with the
+        legacy default stream) instead of using a non-blocking torch stream."""
         import torch
         self.nz_global, self.nv = int(nz_global), int(nv)
         self.bounds = bounds if bounds is not None else [slab_bounds(nz_global, nslabs, r) for r in range(nslabs)]
-        self._streams = [torch.cuda.Stream() for _ in self.bounds]
+        self._streams = [None if blocking_streams else torch.cuda.Stream() for _ in self.bounds]
         self.sims = [B.Cosenu(nzl, nv, L, dt, omega, theta, mu, scheme, use_torch_workspace=False, stream=st,
                               slab=(nz_global, zb), **opts) for (zb, nzl), st in zip(self.bounds, self._streams)]
         for s in self.sims:
@@ -303,8 +306,9 @@ class ConcurrentSlabs(SlabGroup):
             _link(s, peers[lo], peers[hi])
         self._L = self.sims[0]._L
 
-    def step(self, n=1, delays=None):
-        """Every slab's thread enqueues its n steps (4 n launches) on its own stream; delays[r] seconds of head start skew."""
+    def step(self, n=1, delays=None, sync_every_step=None):
+        """Every slab's thread enqueues its n steps (4 n launches) on its own stream; delays[r] seconds of head start skew.
+        sync_every_step[r]: that slab's thread runs step(1) + sync n times instead (a driver that looks at every step)."""
         import threading
         import time
         errs = [None] * len(self.sims)
@@ -313,7 +317,12 @@ class ConcurrentSlabs(SlabGroup):
             try:
                 if delays and delays[r]:
                     time.sleep(delays[r])
-                self.sims[r].step(n)
+                if sync_every_step and sync_every_step[r]:
+                    for _ in range(n):
+                        self.sims[r].step(1)
+                        self.sims[r].sync()
+                else:
+                    self.sims[r].step(n)
             except Exception as e:   # noqa: BLE001  (reported to the caller below)
                 errs[r] = e
 

@@ -231,6 +231,27 @@ def test_free_running_slabs_spin_on_each_other(B, S, scheme, nslabs, skew):
     assert np.array_equal(gotm, refm)
 
 
+@pytest.mark.parametrize("scheme", [FD, FV])
+def test_free_running_slabs_on_blocking_streams(B, S, scheme):
+    """As above, but every handle owns a plain cudaStreamCreate stream (blocking: it synchronises with the legacy default
+    stream), and slab 0's thread looks at every step (step(1) + sync) while slab 1 free-runs.  Nothing the library does
+    between two launches may touch the legacy stream: it would wait for the other slab's queued stages, which spin on the
+    stage this thread has not launched yet, until their halo wait times out (a spurious ESTATE)."""
+    cap = _sm_count() // 2
+    nz, nv = 2 * cap * 16 * 2, 64
+    st = inputs.random_state(nz, nv, seed=911)
+    args = (nz, nv, 0.7 * nz, 0.05, 0.8, 0.3, 1.3, scheme)
+    ref, refm, _ = _single(B, args, st, 12)
+    grp = S.ConcurrentSlabs(2, *args, max_ctas=cap, blocking_streams=True)
+    grp.set_state(st)
+    grp.step(12, sync_every_step=(True, False))
+    grp.sync()
+    got, gotm = grp.get_state(), grp.get_moments()
+    grp.close()
+    assert np.array_equal(got, ref)
+    assert np.array_equal(gotm, refm)
+
+
 def test_missing_neighbour_is_an_error_not_a_hang(B, S):
     """One slab of two steps alone: its waits give up, the flag is raised, and every call that hands results out reports it."""
     nz, nv = 2 * 16 * 8, 32
