@@ -63,12 +63,22 @@ enum {
                               default 3 */
   COSENU_OPT_STAGE_TIMING = 4, /* 1: bracket every stage launch with CUDA events on the handle's stream
                               (read with cosenu_stage_times); default 0 */
-  COSENU_OPT_VARIANT = 5,  /* kernel shape (same arithmetic per cell in all shapes, bit-identical results):
-                              0 (default): FD: 8 compute warps x 2 rows on 16-row tiles.  WENO7 with the default RK form: the marching
-                                 kernel (csrc/weno_march.cuh: one warp per component marches along z through a 16-row tile, separate
-                                 warps combine); WENO7 with the other RK forms: the row-block kernel as in 3;
-                              1: 16 compute warps x 1 row;  2: row-block kernels, WENO7 on 20-24-row tiles with 10-12 compute warps;
-                              3: row-block kernels on 16-row tiles;  4: as 0 */
+  COSENU_OPT_VARIANT = 5,  /* kernel shape (same arithmetic per cell in all shapes, bit-identical results).
+                              FD4+KO: 1: 16 compute warps x 1 row; any other value: 8 compute warps x 2 rows; 16-row tiles always.
+                              WENO7, routing per launch by the KIND of the RK stage (the kinds of RK form 0 are FIRST, MID, MID, LAST;
+                              form 1: FIRST_LEAN, MID_REBUILD, MID, LAST; form 2: FIRST_LEAN, MID_NOACC, MID_NOACC, LAST_COMB;
+                              form 3: FIRST_LEAN, MID_P, MID_NOACC, LAST_P):
+                              0 (default): FIRST_LEAN, MID_P, MID_NOACC and LAST_P -- all of form 3, stage 1 of forms 1 and 2, stages 2, 3
+                                 of form 2 -- run the marching kernel (csrc/weno_march.cuh: one warp per component marches along z
+                                 through a 16-row tile, separate warps combine).  The other kinds run row-block kernels: LAST on 22-row
+                                 tiles when those quantise no worse than 16-row tiles over the persistent grid, on 16-row tiles
+                                 otherwise; FIRST, MID, MID_REBUILD, LAST_COMB always on 16-row tiles.  One RK step of forms 0-2 can
+                                 therefore mix tile heights;
+                              4: as 0 for the four marching kinds; every other kind on 16-row tiles (never the tall ones);
+                              1: row-block kernels, 16 compute warps x 1 row, 16-row tiles, every kind;
+                              2: row-block kernels, every kind; FIRST_LEAN, LAST_P (24 rows, 12 compute warps), MID_NOACC, LAST (22 rows,
+                                 11 warps) and MID_P (20 rows, 10 warps) on tall tiles, the rest on 16-row tiles;
+                              3: row-block kernels, 8 compute warps x 2 rows on 16-row tiles, every kind */
   COSENU_OPT_GRAPH = 8,    /* 1 (default): cosenu_step(n >= 16) replays a CUDA graph of 8 RK4 steps (32 kernel nodes) captured from the
                               handle's own launches, which removes the per-launch host cost on the small, launch-bound grids;
                               0: always launch kernel by kernel.  Not used on slab handles (their launch parameters change every
