@@ -122,7 +122,11 @@ size_t cosenu_workspace_bytes(const cosenu_t* h);
 /* Optional: use caller-owned device memory (>= cosenu_workspace_bytes, 256-byte aligned) and a
  * caller-owned cudaStream_t (NULL: the library creates a blocking stream of its own, which orders with the legacy default
  * stream like default-stream work does).  Must be called before init/set_state;
- * if it never is, the library allocates its own workspace with cudaMalloc on first use. */
+ * if it never is, the library allocates its own workspace with cudaMalloc on first use.
+ * The workspace must be plain DEVICE memory (cudaMalloc / a pooled device allocation: cudaPointerGetAttributes type
+ * cudaMemoryTypeDevice) of the device the handle was created on: the TMA descriptors and the peer stores of the slab
+ * kernels address it directly.  Managed (cudaMallocManaged), pinned-host and pageable memory, and memory of another
+ * device, are refused with COSENU_EINVAL. */
 int cosenu_attach(cosenu_t* h, void* dev_workspace, size_t bytes, void* cuda_stream);
 
 int cosenu_set_option(cosenu_t* h, int key, double value);

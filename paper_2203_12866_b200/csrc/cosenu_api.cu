@@ -110,10 +110,12 @@ int cuda_fail(cosenu* h, cudaError_t e, const char* what) {
   return fail(h, COSENU_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
 }
 // every entry point that touches CUDA runs on the handle's device and leaves the caller's current device as it found it
+// (active = false: an entry point that turns out not to touch CUDA makes no runtime call at all -- cudaGetDevice alone would
+// create a primary context on whatever device the caller has current)
 struct DeviceGuard {
   int prev = -1; bool changed = false;
-  explicit DeviceGuard(int dev) {
-    if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) changed = cudaSetDevice(dev) == cudaSuccess;
+  explicit DeviceGuard(int dev, bool active = true) {
+    if (active && cudaGetDevice(&prev) == cudaSuccess && prev != dev) changed = cudaSetDevice(dev) == cudaSuccess;
   }
   ~DeviceGuard() { if (changed) cudaSetDevice(prev); }
   DeviceGuard(const DeviceGuard&) = delete;
@@ -677,7 +679,8 @@ extern "C" int cosenu_attach(cosenu_t* h, void* dev_workspace, size_t bytes, voi
 
 extern "C" int cosenu_set_option(cosenu_t* h, int key, double value) {
   if (!h) return COSENU_EINVAL;
-  DeviceGuard dg_(h->device);
+  // a pure setter until the handle has touched CUDA: graph, events and tensor maps exist only after ensure_workspace
+  DeviceGuard dg_(h->device, h->maps_ready || h->gexec != nullptr || !h->ev_pool.empty());
   drop_graph(h);   // the captured launch parameters may change
   switch (key) {
     case COSENU_OPT_GRAPH: h->use_graph = value != 0; return COSENU_OK;
