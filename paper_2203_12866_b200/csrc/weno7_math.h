@@ -67,6 +67,12 @@ COSENU_HD double fast_half_rcp(double d) {
 struct Weno7Beam {
   double e0, e1, e2, e3;
 };
+// Host and device builds of this routine are NOT bit-identical: the device forms eps / v^2 from the reciprocal seed plus
+// one third-order step (about 1 ulp), the host divides, so e_r may differ by an ulp or two between them; the host-probe pins
+// (tests/host_probe.cpp) check the formula, tests/device_probe.cu + test_gpu_parity.py::test_device_beam_constants check the
+// device's numbers against eps / v^2 over the accepted range of eps.  Clamping: v^2 below 1e-300 counts as 1e-300 and
+// eps / v^2 above 1e45 as 1e45.  The oracle clamps nothing; the two differ only where (SI + eps/v^2) is eps/v^2 to working
+// precision anyway (weights = d_r, the linear scheme) and the flux carries the factor |v| <= 1e-8.
 COSENU_HD Weno7Beam weno7_beam(double v, double eps) {
   // eps / v^2, kept below 1e45 so that the products of six q_r stay in range for every accepted eps (1e-40 .. 1e30), also
   // on a beam with v = 0 exactly (vertex-centred grids); there the flux is multiplied by |v| = 0 afterwards

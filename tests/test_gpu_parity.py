@@ -455,6 +455,51 @@ def test_marching_kernel_in_a_slab_group_is_bitwise_the_row_block_kernel(B, nsla
     assert np.array_equal(gotm, refm)
 
 
+def test_device_beam_constants(B):
+    """The per-beam constants e_r = (eps / v^2) / sqrt(d_r) as the DEVICE computes them (reciprocal seed + one correction step,
+    csrc/weno7_math.h) against a plain division, over the accepted range of eps and from v = 0 over a tiny non-zero v (the
+    middle beam of a 99-point vertex-centred grid is -1.1e-16, not 0) to |v| = 1, including both clamps."""
+    import ctypes as C
+    import torch
+    import build_probe
+    lib = build_probe.build_device()
+    if lib is None:
+        pytest.skip("no nvcc to build tests/device_probe.cu")
+    P = C.CDLL(lib)
+    P.cosenu_device_probe_weno7_beam.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
+    vmid = float(inputs.v_grid(99, 1)[49])
+    assert vmid != 0.0 and abs(vmid) < 1e-15
+    vs = np.array([0.0, 1e-200, vmid, -vmid, 1e-12, -1e-8, 3e-5, 1.0 / 512, -0.37, 0.99, 1.0, -1.0])
+    es = np.array([1e-40, 1e-30, 1e-6, 1.0, 1e10, 1e30])
+    v, e = [a.ravel().copy() for a in np.meshgrid(vs, es, indexing="ij")]
+    dv, de = torch.from_numpy(v).cuda(), torch.from_numpy(e).cuda()
+    out = torch.full((v.size, 4), float("nan"), dtype=torch.float64, device="cuda")
+    torch.cuda.synchronize()
+    assert P.cosenu_device_probe_weno7_beam(dv.data_ptr(), de.data_ptr(), out.data_ptr(), v.size) == 0
+    got = out.cpu().numpy()
+    with np.errstate(over="ignore"):
+        ev = np.minimum(e / np.maximum(v * v, 1e-300), 1e45)
+    want = ev[:, None] * np.sqrt(35.0 / np.array([4.0, 18.0, 12.0, 1.0]))[None, :]
+    assert np.all(np.isfinite(got))
+    assert np.max(np.abs(got / want - 1.0)) <= 1e-15     # ~4 ulp: seed + step, two roundings of the products
+    assert np.any(ev == 1e45) and np.any(v * v < 1e-300)  # both clamps were exercised
+
+
+@pytest.mark.parametrize("variant", [0, 3])
+@pytest.mark.parametrize("eps", [1e-30, 1e-6, 1e30])
+def test_weno_eps_range_with_a_tiny_nonzero_beam(B, R, eps, variant):
+    """Trapezoid grid with nv = 99: the middle beam is v = -1.1e-16, where the device clamps eps / v^2 (8e61 at eps = 1e30) and
+    the oracle does not; the results agree all the same (the weights are the linear ones on both sides)."""
+    nz, nv = 120, 99
+    assert 0 < abs(inputs.v_grid(nv, 1)[49]) < 1e-15
+    st = inputs.random_state(nz, nv, seed=612)
+    args = (nz, nv, 0.7 * nz, 0.05, 0.8, 0.3, 1.3, FV)
+    got, ref, gm, rm, _, _ = run_pair(B, R, args, st, 2, quadrature=1, weno_eps=eps, variant=variant)
+    assert np.all(np.isfinite(got))
+    assert np.max(np.abs(got - ref)) <= 1e-12 * max(1.0, np.max(np.abs(ref)))
+    assert np.max(np.abs(gm - rm)) <= 1e-12 * max(1.0, np.max(np.abs(rm)))
+
+
 def test_option_ranges_and_attach_validation(B):
     import ctypes as C
     g = B.Cosenu(64, 16, 64.0, 0.1, 0, 0, 1.0, FV)
