@@ -48,18 +48,30 @@ STAGE_KERNEL = {0: ["FIRST", "MID", "MID", "LAST"], 1: ["FIRST_LEAN", "MID_REBUI
 FP64_LANES_PER_CLK = 148 * 4 * 16
 SM_MAX_MHZ = 1965.0
 REPEATS = 3          # repeats of the timed region (best and median of >= 3)
-PROFILE_ROUND = "r02"
+PROFILE_ROUND = "r03"
 
 
 def library_build_id():
-    """sha1 over the sources the library is built from: lets a reader match a bench line to the profile it quotes."""
-    import hashlib
-    h = hashlib.sha1()
-    d = os.path.join(ROOT, "paper_2203_12866_b200", "csrc")
-    for f in sorted(os.listdir(d)) + ["../../include/cosenu.h"]:
-        with open(os.path.join(d, f), "rb") as fh:
-            h.update(fh.read())
-    return h.hexdigest()[:12]
+    """The id compiled into the library that is actually loaded (cosenu_build_id: sha1 over the sources it was built from),
+    so that a stale prebuilt .so cannot carry a fresh id."""
+    from paper_2203_12866_b200 import binding
+    return binding.build_id()
+
+
+def source_build_id():
+    """The same hash over the sources as they sit in the tree right now."""
+    from paper_2203_12866_b200 import build
+    return build.source_id()
+
+
+def profile_build_id():
+    """The library build id the committed ncu capture of this round was taken on (stated in the .md beside the .csv files)."""
+    import re
+    path = os.path.join(ROOT, "profiles", "%s_launches.md" % PROFILE_ROUND)
+    if not os.path.exists(path):
+        return None
+    m = re.search(r"[Ll]ibrary build id[^`]*`([0-9a-f]{12})`", open(path).read())
+    return m.group(1) if m else None
 
 
 def load_profile(workload, rk_form, variant):
@@ -72,6 +84,8 @@ def load_profile(workload, rk_form, variant):
     path = os.path.join(ROOT, "profiles", "%s_metrics_%s.csv" % (PROFILE_ROUND, workload))
     if not os.path.exists(path):
         return None
+    if profile_build_id() != library_build_id():
+        return None     # a capture of another binary is not quoted (roofline.traffic_source says so)
     per = {}
     with open(path) as f:
         rows = list(csv.reader(f))
@@ -309,12 +323,16 @@ def roofline_block(c, rk_form, variant, cells, avg, step_ms, value_per_gpu, cloc
     lead = alu if bound == "alu" else hbm
     r = {"bound": bound, "achieved": lead["achieved"], "peak": lead["peak"], "unit": lead["unit"], "frac": lead["frac"],
          "traffic": per_stage[dom].get("ncu_dram_bytes"),
-         "traffic_source": (prof["file"] + " (ncu, same command as this bench line; library build id in the .md beside it)") if prof else None,
+         "traffic_source": (prof["file"] + " (committed ncu capture of `bench.py --workload %s --steps 2 --warmup 5 --no-cpu-baseline "
+                            "--no-secondary --e2e-steps 1` on the same library build, not measured in this run; full command in "
+                            "profiles/%s_launches.md)" % (c["name"], PROFILE_ROUND)) if prof else
+                           ("none: profiles/%s_launches.md was captured on library build %s, the loaded library is %s"
+                            % (PROFILE_ROUND, profile_build_id(), library_build_id())),
          "kernel": "%s (RK stage %d, %s)" % (prof["stages"][dom]["kernel"] if prof else "stage kernel", dom + 1, names[dom]),
          "avg_launch_ms": avg[dom], "stage_kernel_share_of_step": sum(avg) / step_ms,
          "hbm": hbm, "alu": alu, "per_stage": per_stage, "bytes_per_cell_step": sum(sb),
          "step_GBps": sum(sb) * value_per_gpu / 1e9, "step_frac_of_hbm_peak": sum(sb) * value_per_gpu / 1e9 / peak,
-         "library_build_id": library_build_id()}
+         "library_build_id": library_build_id(), "library_matches_sources": library_build_id() == source_build_id()}
     return r
 
 
@@ -543,7 +561,10 @@ def run_ours(args):
     out = {"metric": METRIC, "value": main_r["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": main_r["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "f64", "data": "synthetic", "config": config_of(main_r, args, world, decomp),
-           "timing": "median of %d repeats of the timed region of K steps; best in `repeats`" % REPEATS, "repeats": main_r["repeats"],
+           "timing": "median of %d repeats of the timed region of K steps; the per-stage CUDA events (COSENU_OPT_STAGE_TIMING, five event "
+                     "records per step on the launching stream, launch by launch, no CUDA-graph replay) are ON inside it; the first "
+                     "repeat is usually the fastest (the board's power controller), all are in `repeats`; `graph_replay` is the same "
+                     "workload replayed from a CUDA graph without events" % REPEATS, "repeats": main_r["repeats"],
            "clocks": main_r["clocks"], "e2e": main_r["e2e"], "gpu_launches": main_r["launches"], "roofline": main_r["roofline"],
            "cpu_baseline": cpu, "graph_replay": main_r["graph_replay"], "checks": main_r["checks"], "secondary": secondary}
     if world > 1:

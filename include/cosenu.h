@@ -172,6 +172,11 @@ int cosenu_stage_times(cosenu_t* h, double* ms_sum, int64_t* launches_per_stage)
 void cosenu_destroy(cosenu_t* h);
 const char* cosenu_last_error(const cosenu_t* h);
 
+/* Identity of the loaded binary: the first 12 hex digits of the sha1 over the sources it was compiled from (csrc/ in
+ * name order, then this header), put in at compile time by paper_2203_12866_b200/build.py ("unknown" for a build made by
+ * hand).  bench.py prints it, and quotes an ncu capture under profiles/ only if the capture names the same id. */
+const char* cosenu_build_id(void);
+
 /* ===================================================================================================
  * z-slab decomposition over several GPUs (the paper's "future work").
  *

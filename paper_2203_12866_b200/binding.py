@@ -24,7 +24,7 @@ SYMBOLS = ["cosenu_create", "cosenu_workspace_bytes", "cosenu_attach", "cosenu_s
            "cosenu_create_slab", "cosenu_slab_export", "cosenu_slab_link", "cosenu_slab_push_ghosts",
            "cosenu_slab_ref_sums", "cosenu_slab_set_ref_sums", "cosenu_slab_diag_sums", "cosenu_slab_diag_finish",
            "cosenu_slab_step_group", "cosenu_slab_stage", "cosenu_slab_wait_failed",
-           "cosenu_beam_sums_static", "cosenu_beam_sums_static_error"]
+           "cosenu_beam_sums_static", "cosenu_beam_sums_static_error", "cosenu_build_id"]
 STATIC_MAX_NV = 512   # COSENU_STATIC_MAX_NV of include/cosenu.h
 
 
@@ -97,8 +97,15 @@ def load():
     L.cosenu_beam_sums_static.argtypes = [C.c_void_p, C.c_int64, C.c_int32, C.c_void_p, C.c_void_p]
     L.cosenu_beam_sums_static_error.restype = C.c_char_p
     L.cosenu_beam_sums_static_error.argtypes = []
+    L.cosenu_build_id.restype = C.c_char_p
+    L.cosenu_build_id.argtypes = []
     _lib = L
     return L
+
+
+def build_id():
+    """cosenu_build_id: the source hash compiled into the loaded library."""
+    return load().cosenu_build_id().decode()
 
 
 class CosenuError(RuntimeError):

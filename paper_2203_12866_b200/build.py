@@ -22,6 +22,19 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", 
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
 
 
+def source_id():
+    """sha1 (12 hex digits) over the sources the library is built from, in a fixed order.  Compiled into the library
+    (cosenu_build_id) so that a bench line and an ncu capture can name the binary they ran, not the tree they sat in."""
+    import hashlib
+    h = hashlib.sha1()
+    for f in sorted(os.listdir(CSRC)):
+        with open(os.path.join(CSRC, f), "rb") as fh:
+            h.update(fh.read())
+    with open(os.path.join(ROOT, "include", "cosenu.h"), "rb") as fh:
+        h.update(fh.read())
+    return h.hexdigest()[:12]
+
+
 def _newer(out, deps):
     return os.path.exists(out) and all(os.path.getmtime(out) >= os.path.getmtime(d) for d in deps)
 
@@ -31,7 +44,7 @@ def build(force=False, verbose=False):
     deps = srcs + [os.path.join(ROOT, "include", "cosenu.h"), os.path.abspath(__file__)]
     if force or not _newer(LIB, deps):
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+        cmd = [nvcc] + NVCC_FLAGS + ['-DCOSENU_BUILD_ID="%s"' % source_id()] + (["-Xptxas", "-v"] if verbose else []) + \
               ["-o", LIB] + [os.path.join(CSRC, f) for f in UNITS]
         subprocess.run(cmd, check=True)
     return LIB

@@ -884,6 +884,11 @@ extern "C" void cosenu_destroy(cosenu_t* h) {
 
 extern "C" const char* cosenu_last_error(const cosenu_t* h) { return h ? h->err.c_str() : g_create_err.c_str(); }
 
+#ifndef COSENU_BUILD_ID
+#define COSENU_BUILD_ID "unknown"   // built by hand, without paper_2203_12866_b200/build.py
+#endif
+extern "C" const char* cosenu_build_id(void) { return COSENU_BUILD_ID; }
+
 // ================================================================================ z-slab decomposition
 namespace {
 typedef CUresult (*PFN_getAddressRange)(CUdeviceptr*, size_t*, CUdeviceptr);
