@@ -44,6 +44,27 @@ __global__ void push_ghosts_kernel(const double* __restrict__ y, long long nz, i
   }
 }
 
+// cosenu_init on the device: the initial state is an outer product -- every entry is ONE product of a per-beam number
+// (Eq. 20: g_nu(v_j), alpha g_nubar(v_j), normalised on the host) and a per-row number (the seeded phase or
+// Eq. 21's Gaussian, evaluated on the host: O(nz + nv) libm calls in all).  The host uploads
+// zv[4][nz] = (1 + d, 1 - d, Re, Im) and gv[2][nv] = (g, gbar) and this kernel forms the 8 planes, each entry with the same
+// single rounding the host loop used to make ((g * 0.5) is exact), so the state is bit-identical to the old host expansion.
+__global__ void init_expand_kernel(double* __restrict__ y, const double* __restrict__ zv, const double* __restrict__ gv,
+                                   long long nz, int nv, int nvp, long long comp_stride, int g) {
+  for (long long iz = blockIdx.x; iz < nz; iz += gridDim.x) {
+    const double ap = zv[iz], am = zv[nz + iz], pr = zv[2 * nz + iz], pi = zv[3 * nz + iz];
+    double* row = y + (iz + g) * nvp;
+    for (int j = threadIdx.x; j < nv; j += blockDim.x) {
+      const double gj = gv[j], gbj = gv[nv + j];
+      const double hg = __dmul_rn(gj, 0.5), hgb = __dmul_rn(gbj, 0.5);
+      row[j] = __dmul_rn(hg, ap);                     row[comp_stride + j] = __dmul_rn(hg, am);
+      row[2 * comp_stride + j] = __dmul_rn(gj, pr);   row[3 * comp_stride + j] = __dmul_rn(gj, pi);
+      row[4 * comp_stride + j] = __dmul_rn(hgb, ap);  row[5 * comp_stride + j] = __dmul_rn(hgb, am);
+      row[6 * comp_stride + j] = __dmul_rn(gbj, pr);  row[7 * comp_stride + j] = __dmul_rn(gbj, pi);
+    }
+  }
+}
+
 // the 6 velocity moments per z of a state (S1; Riemann sum of PAPER.md:78): one warp per z row,
 // lanes stride over v, fixed shuffle tree => reproducible.  mom[6][nz], already times dv.
 __global__ void moments_kernel(const double* __restrict__ y, double* __restrict__ mom, long long nz, int nv, int nvp,

@@ -735,8 +735,6 @@ extern "C" int cosenu_init(cosenu_t* h, uint64_t seed, double sigma_nu, double s
   if (!(sigma_nu > 0) || !(sigma_nubar > 0) || !(alpha >= 0) || !std::isfinite(pert_amp) || pert_kind < 0 || pert_kind > 2)
     return fail(h, COSENU_EINVAL, "cosenu_init: invalid argument");
   const int nv = h->nv; const int64_t nz = h->nz;
-  std::vector<double> st;
-  try { st.assign(8 * (size_t)nz * nv, 0.0); } catch (...) { return fail(h, COSENU_ENOMEM, "cosenu_init: host out of memory"); }
   // Eq. (20), normalised so that sum_j g_j dv = 1; g_bar carries alpha
   std::vector<double> g(nv), gb(nv);
   double sg = 0, sgb = 0;
@@ -776,16 +774,29 @@ extern "C" int cosenu_init(cosenu_t* h, uint64_t seed, double sigma_nu, double s
       pr[i] = 0.5 * e; pi[i] = 0.0; dd[i] = std::sqrt(1.0 - e * e);
     }
   }
-  const size_t pl = (size_t)nz * nv;
-  for (int64_t i = 0; i < nz; ++i)
-    for (int j = 0; j < nv; ++j) {
-      const size_t q = (size_t)i * nv + j;
-      st[0 * pl + q] = g[j] * 0.5 * (1.0 + dd[i]);  st[1 * pl + q] = g[j] * 0.5 * (1.0 - dd[i]);
-      st[2 * pl + q] = g[j] * pr[i];                st[3 * pl + q] = g[j] * pi[i];
-      st[4 * pl + q] = gb[j] * 0.5 * (1.0 + dd[i]); st[5 * pl + q] = gb[j] * 0.5 * (1.0 - dd[i]);
-      st[6 * pl + q] = gb[j] * pr[i];               st[7 * pl + q] = gb[j] * pi[i];
-    }
-  return cosenu_set_state(h, st.data(), 0.0);
+  // The state is the outer product of these vectors: the host holds O(nz + nv) numbers and the device expands them
+  // (init_expand_kernel; each entry one product, rounded once, exactly as a host loop over all cells would).
+  // Scratch on the device: the 4 nz-vectors go into the moment buffer that the first stage launch overwrites, the 2
+  // nv-vectors into the diagnostics partials that finish_upload overwrites.
+  std::vector<double> zv(4 * (size_t)nz), gv(2 * (size_t)nv);
+  for (int64_t i = 0; i < nz; ++i) {
+    zv[i] = 1.0 + dd[i]; zv[(size_t)nz + i] = 1.0 - dd[i]; zv[2 * (size_t)nz + i] = pr[i]; zv[3 * (size_t)nz + i] = pi[i];
+  }
+  for (int j = 0; j < nv; ++j) { gv[j] = g[j]; gv[(size_t)nv + j] = gb[j]; }
+  DeviceGuard dg_(h->device);
+  int rc = ensure_workspace(h);
+  if (rc) return rc;
+  double* d_zv = h->M[1];
+  double* d_gv = h->d_refpart;
+  static_assert(REF_BLOCKS * 4 >= 2, "the diagnostics partials hold the two beam vectors");
+  CK(cudaMemcpyAsync(d_zv, zv.data(), sizeof(double) * zv.size(), cudaMemcpyHostToDevice, h->stream));
+  CK(cudaMemcpyAsync(d_gv, gv.data(), sizeof(double) * gv.size(), cudaMemcpyHostToDevice, h->stream));
+  const unsigned blocks = (unsigned)(nz < 4 * (int64_t)h->num_sms * 8 ? nz : 4 * (int64_t)h->num_sms * 8);
+  init_expand_kernel<<<blocks, 256, 0, h->stream>>>(h->U, d_zv, d_gv, nz, nv, h->nvp, h->comp_stride, G);
+  CK(cudaGetLastError());
+  h->launches++;
+  rc = finish_upload(h, 0.0);     // synchronises the stream: zv / gv are no longer needed when it returns
+  return rc;
 }
 
 extern "C" int cosenu_step(cosenu_t* h, int64_t n) {

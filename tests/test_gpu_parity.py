@@ -239,6 +239,46 @@ def test_init_matches_oracle_init(B, R):
                                rtol=1e-14, atol=1e-21)
 
 
+_INIT_COST_SCRIPT = r"""
+import json, resource, sys, time
+sys.path.insert(0, %r)
+import torch
+from paper_2203_12866_b200 import binding as B, inputs
+c = inputs.CONFIGS["cfg4"]
+g = B.Cosenu(c["nz"], c["nv"], c["L"], c["dt"], c["omega"], c["theta"], c["mu"], c["scheme"])
+g.init(c["seed"])                                   # first call: workspace set-up, kernel loading
+torch.cuda.synchronize()
+rss0 = resource.getrusage(resource.RUSAGE_SELF).ru_maxrss
+t0 = time.perf_counter()
+g.init(c["seed"] + 1)
+dt = time.perf_counter() - t0
+rss1 = resource.getrusage(resource.RUSAGE_SELF).ru_maxrss
+d = g.diagnostics()
+print(json.dumps({"seconds": dt, "peak_rss_growth_kb": rss1 - rss0, "psurv_nu": d["psurv_nu"]}))
+"""
+
+
+def test_cfg4_init_costs_the_host_next_to_nothing(B):
+    """cosenu_init holds O(nz + nv) numbers on the host and expands them on the device: at 262144 x 512 (an 8.6 GB state) a
+    call takes under 100 ms of wall time and grows the process's peak resident set by under 10 MB (it used to build the
+    8.6 GB state in a std::vector first).  Measured in a fresh process, where the peak is not already set by other tests."""
+    import json
+    import os
+    import subprocess
+    import sys
+    import torch
+    free, _ = torch.cuda.mem_get_info()
+    if free < 40e9:
+        pytest.skip("needs 35 GB of device memory")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, "-c", _INIT_COST_SCRIPT % root], capture_output=True, text=True, timeout=300)
+    assert out.returncode == 0, out.stderr[-2000:]
+    r = json.loads(out.stdout.strip().splitlines()[-1])
+    assert r["seconds"] < 0.1, r
+    assert r["peak_rss_growth_kb"] < 10 * 1024, r
+    assert abs(r["psurv_nu"] - 1.0) < 1e-12, r
+
+
 def _init_state(B, nz, nv, seed):
     g = B.Cosenu(nz, nv, float(nz), 0.4, 0.0, 0.0, 1.0, FD)
     g.init(seed)
@@ -392,6 +432,56 @@ def test_full_size_cfg4_windows(B, R):
     assert d["trace_dev_max"] <= 1e-12
     s2, c2 = np.sin(2 * c["theta"]), np.cos(2 * c["theta"])
     assert abs(s2 * d["dM0"][0] - c2 * d["dM0"][2]) <= 1e-9 * c["nz"]
+
+
+def _gate_windows(name, nrand, seed):
+    """Windows for the 20-step gate at a bandwidth-scale config: `nrand` seeded-random ones plus forced ones where an indexing
+    slip of the persistent tile walk would sit: the periodic seam (last tile of the grid | tile 0), and the rows where the LAST
+    tile of the last CTA's walk meets the LAST tile of CTA 0's walk (CTA b walks the 16-row tiles b, b + n_sm, b + 2 n_sm, ...)."""
+    import torch
+    c = inputs.CONFIGS[name]
+    nz = c["nz"]
+    nsm = torch.cuda.get_device_properties(0).multi_processor_count
+    ntiles = (nz + 15) // 16
+    last0 = (ntiles - 1) // nsm * nsm                      # CTA 0's last tile; tile last0 - 1 is CTA (nsm - 1)'s last one
+    rng = np.random.default_rng(seed)
+    wins = [(int(z), int(w)) for z, w in zip(rng.integers(0, nz, nrand), rng.integers(4, 9, nrand))]
+    wins += [(nz - 3, 6), (last0 * 16 - 4, 8), (last0 * 16 + 12, 8), ((nsm - 1) * 16 + 12, 8)]   # ..., tile of the last CTA | CTA 0's second tile
+    return wins
+
+
+@pytest.mark.parametrize("name", ["cfg3", "cfg4"])
+def test_full_size_gate_20_steps(B, R, name):
+    """BASELINE north_star's gate, at the two bandwidth-scale configs it names and in the launch configuration bench.py times:
+    after 20 RK4 steps every element of 32 seeded-random windows and 4 forced ones (about 230 rows x N_v x 8 components per
+    config) is within 1e-12 of the oracle, which advances each window with a margin of 16 * 20 + 4 rows per side (the domain
+    of dependence of 20 steps: 4 stages x 4 rows)."""
+    import torch
+    free, _ = torch.cuda.mem_get_info()
+    if name == "cfg4" and free < 40e9:
+        pytest.skip("needs 35 GB of device memory")
+    _window_parity(B, R, name, 20, _gate_windows(name, 32, 20220312), TOL20)
+
+
+def test_full_size_cfg3_self_linked_slab_is_bitwise_the_single_domain(B):
+    """A slab handle walks its tiles edge tiles first (tile_shift = ntiles - 2: the walk wraps after its second tile).  One slab
+    that is the whole cfg3 grid, linked to itself, must give the single domain's bits at full size, wrap included."""
+    from paper_2203_12866_b200 import slab as S
+    c = inputs.CONFIGS["cfg3"]
+    args = (c["nz"], c["nv"], c["L"], c["dt"], c["omega"], c["theta"], c["mu"], c["scheme"])
+    st = inputs.config_state("cfg3")
+    g = B.Cosenu(*args)
+    g.set_state(st)
+    g.step(3)
+    ref = g.get_state()
+    g.close()
+    grp = S.SlabGroup(1, *args)
+    grp.set_state(st)
+    grp.step(3)
+    grp.sync()
+    got = grp.get_state()
+    grp.close()
+    assert np.array_equal(got, ref)
 
 
 @pytest.mark.parametrize("variant", [0, 3])
