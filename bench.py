@@ -373,9 +373,12 @@ def bench_workload(args, name, steps, warmup, world, rank, local, decomp, e2e_st
         from paper_2203_12866_b200 import slab as S
         sim = S.CosenuSlab(world * nz, nv, world * c["L"], c["dt"], c["omega"], c["theta"], c["mu"], c["scheme"],
                            rk_form=args.rk_form, variant=args.variant)
+        api = sim.sim
+        # ranks reach their first step at different times (uploads, the e2e leg's 8.6 GB copies): a halo wait that gives up
+        # after the default 4 s would turn one slow rank into "halo_wait_failed"
+        api.set_option(B.OPT_HALO_TIMEOUT_S, 60.0)
         sim.init(c["seed"])
         sim.get_state(host)
-        api = sim.sim
     else:
         sim = B.Cosenu(nz, nv, c["L"], c["dt"], c["omega"], c["theta"], c["mu"], c["scheme"], rk_form=args.rk_form,
                        variant=args.variant)
@@ -383,6 +386,7 @@ def bench_workload(args, name, steps, warmup, world, rank, local, decomp, e2e_st
         api = sim
 
     # ---- device-resident throughput: W warm-up steps, then REPEATS timed regions of exactly K steps
+    barrier()            # every rank holds its state (and, decomposed, its neighbours' ghost rows) before anybody steps
     sim.step(warmup)
     barrier()
     sampler = ClockSampler(local) if (sample_clocks and rank == 0) else None
@@ -446,7 +450,9 @@ def config_of(r, args, world, decomp):
             "dt": c["dt"], "omega": c["omega"], "theta": c["theta"], "mu": c["mu"],
             "state_bytes_per_copy": 8 * r["cells"] * 8, "l2": "inputs larger than L2 (no flush needed)" if r["cells"] * 64 > 4 * 126e6
             else "state of %.1f MB fits in L2: launch-bound grid, reported in `secondary` only" % (r["cells"] * 64 / 1e6),
-            "parallelism": ("z-slabs x%d of one grid of %d rows (halo exchange fused into the stage kernels)"
+            "parallelism": ("z-slabs x%d of one grid of %d rows (halo exchange fused into the stage kernels: the data plane is "
+                            "peer-memory stores + arrival counters over NVLink, NOT NCCL; torch.distributed/NCCL carries only the "
+                            "set-up descriptors, the diagnostics' few sums and the barriers)"
                             % (world, world * c["nz"])) if decomp == "slab" else "replicas x%d" % world,
             "rk_form": args.rk_form, "variant": args.variant}
 

@@ -86,6 +86,9 @@ enum {
   COSENU_OPT_MAX_CTAS = 9, /* cap of the persistent grid of a stage launch (0, default: one CTA per SM).  With a cap of at most half the SMs
                               the stage kernels of two slab handles driven from two streams are co-resident, which is how the fused
                               halo exchange is exercised on one GPU (tests/test_gpu_slab.py); no other use */
+  COSENU_OPT_HALO_TIMEOUT_S = 10, /* z-slab handles: seconds a stage kernel waits for a neighbour's ghost rows before it gives up and
+                              flags the run invalid (cosenu_slab_wait_failed); default 4, 0.001 .. 3600.  Raise it where ranks may
+                              start a step far apart (a first step after a slow upload on one rank, a debugger, a loaded node). */
   COSENU_OPT_KO_ORDER = 7, /* r of the Kreiss-Oliger operator of Eq. (5): 2 (default; "r = 2 for most numerical
                               experiments"; 5-point, halo 2) or 3 (7-point (eps/64dz) delta^6, halo 3).  FD scheme only;
                               the handle's stream is idle when this is changed. */
@@ -252,7 +255,8 @@ int cosenu_slab_step_group(cosenu_t** hs, int32_t count, int64_t n);
  * for a kernel of another process: sync + barrier after every stage, so every counter has arrived before the launch. */
 int cosenu_slab_stage(cosenu_t* h, int32_t k);
 
-/* 1 if a halo wait of this handle ever timed out (a neighbour did not arrive within ~4 s); synchronises. */
+/* 1 if a halo wait of this handle ever timed out (a neighbour did not arrive within COSENU_OPT_HALO_TIMEOUT_S, default 4 s);
+ * synchronises. */
 int cosenu_slab_wait_failed(cosenu_t* h, int32_t* failed);
 
 /* ===================================================================================================

@@ -16,6 +16,7 @@ FD4_KO3, FV_WENO7 = 0, 1
 OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, 1, 2, 3, 4
 OPT_EPS_KO, OPT_WENO_EPS, OPT_ADVECT, OPT_RK_FORM, OPT_STAGE_TIMING, OPT_VARIANT, OPT_QUADRATURE, OPT_KO_ORDER, OPT_GRAPH = 0, 1, 2, 3, 4, 5, 6, 7, 8
 OPT_MAX_CTAS = 9
+OPT_HALO_TIMEOUT_S = 10
 
 # every symbol include/cosenu.h declares
 SYMBOLS = ["cosenu_create", "cosenu_workspace_bytes", "cosenu_attach", "cosenu_set_option", "cosenu_init",

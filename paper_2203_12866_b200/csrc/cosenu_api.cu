@@ -53,6 +53,7 @@ struct cosenu {
   int variant = 0;       // kernel shape variant (COSENU_OPT_VARIANT)
   int num_sms = 148;
   int max_ctas = 0;      // COSENU_OPT_MAX_CTAS: cap of the persistent grid of a stage launch (0: one CTA per SM)
+  double halo_timeout_s = 4.0;   // COSENU_OPT_HALO_TIMEOUT_S: how long a slab's halo wait may last
 
   // workspace
   void* ws = nullptr; size_t ws_bytes = 0; bool ws_owned = false;
@@ -411,6 +412,7 @@ void set_output(cosenu* h, StageParams& p, int which) {
   p.wait_hi = h->d_ctr + 1;
   p.wait_val = (unsigned long long)G * h->epoch;   // G rows per edge per stage launch so far
   p.err_flag = h->d_err;
+  p.wait_timeout_ns = (unsigned long long)(h->halo_timeout_s * 1e9);
 }
 
 // RK stage k (0..3) of the classical RK4 step = ONE fused launch.  Buffers: U -> Y1 -> Y2 -> (Y1 | ACC) -> U; in the
@@ -687,6 +689,7 @@ extern "C" int cosenu_set_option(cosenu_t* h, int key, double value) {
     case COSENU_OPT_EPS_KO: if (!(value >= 0) || !std::isfinite(value)) break; h->eps_ko = value; return COSENU_OK;
     case COSENU_OPT_WENO_EPS: if (!(value >= 1e-40) || !(value <= 1e30)) break; h->weno_eps = value; return COSENU_OK;   // range of the product form, weno7_math.h
     case COSENU_OPT_MAX_CTAS: if (!(value >= 0) || !(value <= 65535) || value != std::floor(value)) break; h->max_ctas = (int)value; return COSENU_OK;
+    case COSENU_OPT_HALO_TIMEOUT_S: if (!(value >= 1e-3) || !(value <= 3600.0)) break; h->halo_timeout_s = value; return COSENU_OK;
     case COSENU_OPT_ADVECT: h->advect = value != 0; return COSENU_OK;
     case COSENU_OPT_RK_FORM: if (value != 0 && value != 1 && value != 2 && value != 3) break; h->rk_form = (int)value; return COSENU_OK;
     case COSENU_OPT_VARIANT: if (value != 0 && value != 1 && value != 2 && value != 3 && value != 4) break; h->variant = (int)value; return COSENU_OK;

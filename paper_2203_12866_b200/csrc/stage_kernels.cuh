@@ -80,6 +80,7 @@ struct StageParams {
   const unsigned long long* wait_hi;
   unsigned long long wait_val;
   int* err_flag;           // set to 1 when a wait gives up (a neighbour that never arrives must not hang the GPU)
+  unsigned long long wait_timeout_ns;   // how long a halo wait may last before it gives up (COSENU_OPT_HALO_TIMEOUT_S)
   long long tile_shift;    // the l-th tile a CTA grid walks is tile (l + tile_shift) mod ntiles (slab: edge tiles first)
 };
 
@@ -148,14 +149,15 @@ __device__ __forceinline__ unsigned long long global_timer_ns() {
   asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
   return t;
 }
-// wait until *ctr >= val; gives up after ~4 s (sets *err) so that a missing neighbour is an error, not a hang
-__device__ __noinline__ void wait_arrivals(const unsigned long long* ctr, unsigned long long val, int* err) {
+// wait until *ctr >= val; gives up after timeout_ns (default 4 s; sets *err) so that a missing neighbour is an error, not a hang
+__device__ __noinline__ void wait_arrivals(const unsigned long long* ctr, unsigned long long val, int* err,
+                                           unsigned long long timeout_ns) {
   if (ld_acquire_sys(ctr) >= val) return;
-  if (err && *reinterpret_cast<volatile int*>(err)) return;   // an earlier wait has already given up: the run is invalid, do not add 4 s per tile
+  if (err && *reinterpret_cast<volatile int*>(err)) return;   // an earlier wait has already given up: the run is invalid, do not add the time-out per tile
   const unsigned long long t0 = global_timer_ns();
   while (ld_acquire_sys(ctr) < val) {
     __nanosleep(200);
-    if (global_timer_ns() - t0 > 4000000000ull) {
+    if (global_timer_ns() - t0 > timeout_ns) {
       if (err) atomicExch(err, 1);
       return;
     }
@@ -361,8 +363,8 @@ __global__ void __launch_bounds__(NSEG * 32 + 32, 1)
           // z-slab: the ghost rows this tile reads (and the neighbour's ghost rows its edge rows overwrite) belong to
           // the exchange with the neighbouring GPUs: wait for their rows of the previous stage
           bool waited = false;
-          if (p.wait_lo != nullptr && tile * TZ < G) { wait_arrivals(p.wait_lo, p.wait_val, p.err_flag); waited = true; }
-          if (p.wait_hi != nullptr && (tile + 1) * TZ + G > p.nz) { wait_arrivals(p.wait_hi, p.wait_val, p.err_flag); waited = true; }
+          if (p.wait_lo != nullptr && tile * TZ < G) { wait_arrivals(p.wait_lo, p.wait_val, p.err_flag, p.wait_timeout_ns); waited = true; }
+          if (p.wait_hi != nullptr && (tile + 1) * TZ + G > p.nz) { wait_arrivals(p.wait_hi, p.wait_val, p.err_flag, p.wait_timeout_ns); waited = true; }
           if (waited) asm volatile("fence.proxy.async.global;" ::: "memory");   // generic-proxy acquire -> TMA (async proxy) reads
         }
         mbar_wait(b_empty_y + 8 * sy, (uint32_t)(((n / NY) & 1) ^ 1));

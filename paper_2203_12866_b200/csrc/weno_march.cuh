@@ -195,8 +195,8 @@ __global__ void __launch_bounds__(MARCH_THREADS, 1)
         const int sy = (int)(n & 1), su = sy;
         if (ch == 0 && (p.wait_lo != nullptr || p.wait_hi != nullptr)) {
           bool waited = false;
-          if (p.wait_lo != nullptr && tile * TZ < G) { wait_arrivals(p.wait_lo, p.wait_val, p.err_flag); waited = true; }
-          if (p.wait_hi != nullptr && (tile + 1) * TZ + G > p.nz) { wait_arrivals(p.wait_hi, p.wait_val, p.err_flag); waited = true; }
+          if (p.wait_lo != nullptr && tile * TZ < G) { wait_arrivals(p.wait_lo, p.wait_val, p.err_flag, p.wait_timeout_ns); waited = true; }
+          if (p.wait_hi != nullptr && (tile + 1) * TZ + G > p.nz) { wait_arrivals(p.wait_hi, p.wait_val, p.err_flag, p.wait_timeout_ns); waited = true; }
           if (waited) asm volatile("fence.proxy.async.global;" ::: "memory");
         }
         mbar_wait(b_empty_y + 8 * sy, (uint32_t)(((n >> 1) & 1) ^ 1));

@@ -269,6 +269,28 @@ def test_missing_neighbour_is_an_error_not_a_hang(B, S):
     grp.sims = []
 
 
+def test_halo_timeout_is_an_option(B, S):
+    """COSENU_OPT_HALO_TIMEOUT_S: with 0.5 s a slab whose neighbour never steps is flagged well before the default 4 s."""
+    import time
+    nz, nv = 2 * 16 * 8, 32
+    grp = S.ConcurrentSlabs(2, nz, nv, 0.7 * nz, 0.05, 0.8, 0.3, 1.3, FV, max_ctas=8)
+    for s in grp.sims:
+        s.set_option(B.OPT_HALO_TIMEOUT_S, 0.5)
+    for bad in (0.0, -1.0, 1e6, float("nan")):
+        with pytest.raises(B.CosenuError):
+            grp.sims[0].set_option(B.OPT_HALO_TIMEOUT_S, bad)
+    grp.set_state(inputs.random_state(nz, nv, seed=78))
+    t0 = time.perf_counter()
+    grp.sims[0].step(1)
+    with pytest.raises(B.CosenuError):
+        grp.sims[0].sync()
+    assert time.perf_counter() - t0 < 3.0
+    assert S._wait_failed(grp.sims[0])
+    for s in grp.sims:
+        s.close()
+    grp.sims = []
+
+
 def test_two_gpus_free_running(B, S):
     """Two slabs on two GPUs of this process (peer access), free-running: needs a box with at least two devices."""
     import torch
