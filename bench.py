@@ -11,7 +11,7 @@ L2, so no L2 flush is needed between steps.  The timed region of K steps is repe
 the best is in `repeats`.  The same line carries `secondary`: the bandwidth-scale FD4+KO3 run (cfg3, with its own
 roofline and clocks) and the launch-bound grids cfg0-cfg2 (ms per step launch by launch and as CUDA-graph replays).
 `roofline` leads with what binds the dominant launch ("alu": the plain fp64 pipe, WENO7; "hbm": FD4+KO3); the per-stage
-ncu counters it quotes (DRAM bytes, fp64 instructions) are read from the committed capture profiles/r02_metrics_*.csv.
+ncu counters it quotes (DRAM bytes, fp64 instructions) are read from the committed capture profiles/r03_metrics_*.csv.
 
 N > 1 (torchrun): ONE periodic grid of N x nz rows cut into z-slabs, one per rank: the halo exchange is fused into
 the stage kernels (peer stores over NVLink + arrival counters); weak scaling (nz rows per
