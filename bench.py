@@ -325,9 +325,12 @@ def roofline_block(c, rk_form, variant, cells, avg, step_ms, value_per_gpu, cloc
          "traffic": per_stage[dom].get("ncu_dram_bytes"),
          "traffic_source": (prof["file"] + " (committed ncu capture of `bench.py --workload %s --steps 2 --warmup 5 --no-cpu-baseline "
                             "--no-secondary --e2e-steps 1` on the same library build, not measured in this run; full command in "
-                            "profiles/%s_launches.md)" % (c["name"], PROFILE_ROUND)) if prof else
-                           ("none: profiles/%s_launches.md was captured on library build %s, the loaded library is %s"
-                            % (PROFILE_ROUND, profile_build_id(), library_build_id())),
+                            "profiles/%s_launches.md)" % (c["name"], PROFILE_ROUND)) if prof else None,
+         # a committed capture of this workload exists but names another binary: it is not quoted, and this says why
+         "traffic_not_quoted": ("profiles/%s_launches.md was captured on library build %s, the loaded library is %s"
+                                % (PROFILE_ROUND, profile_build_id(), library_build_id()))
+         if (prof is None and rk_form == 3 and variant in (0, 4) and profile_build_id() != library_build_id()
+             and os.path.exists(os.path.join(ROOT, "profiles", "%s_metrics_%s.csv" % (PROFILE_ROUND, c["name"])))) else None,
          "kernel": "%s (RK stage %d, %s)" % (prof["stages"][dom]["kernel"] if prof else "stage kernel", dom + 1, names[dom]),
          "avg_launch_ms": avg[dom], "stage_kernel_share_of_step": sum(avg) / step_ms,
          "hbm": hbm, "alu": alu, "per_stage": per_stage, "bytes_per_cell_step": sum(sb),
